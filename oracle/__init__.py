@@ -1,0 +1,155 @@
+"""CPU oracle for the Chorus II sparsity-reuse hot path — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Thin ctypes binding over ``oracle/chorus_oracle.cpp`` (plain fp64 C++, written from the paper; see
+the header of that file for citations and pin status).  Only ``tests/``, ``__graft_entry__.smoke()``
+and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import this package.  It imports
+nothing from ``paper_2606_25040_b200`` and the CUDA path imports nothing from here.
+
+All arrays are numpy: bf16 tensors travel as ``uint16`` bit patterns, e4m3 tensors as ``uint8`` codes.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from .build import build as _build
+
+BQ, BK = 128, 64
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        _lib.oracle_mask_to_index.restype = C.c_int64
+        _lib.oracle_e4m3_to_double.restype = C.c_double
+        _lib.oracle_e4m3_to_double.argtypes = [C.c_uint8]
+        _lib.oracle_float_to_e4m3.restype = C.c_uint8
+        _lib.oracle_float_to_e4m3.argtypes = [C.c_float]
+        _lib.oracle_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _c(a, dtype):
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def mask_to_index(bitmask: np.ndarray, nk: int, count_only: bool = False):
+    """bitmask uint32 [L][H][nq][words] -> (row_ptr int32 [L*H*nq+1], col_idx int32 [nnz])."""
+    bm = _c(bitmask, np.uint32)
+    L, H, nq, words = bm.shape
+    assert words == (nk + 31) // 32
+    row_ptr = np.zeros(L * H * nq + 1, dtype=np.int32)
+    nnz = lib().oracle_mask_to_index(_p(bm), L, H, nq, nk, _p(row_ptr), None)
+    if count_only:
+        return row_ptr, None
+    col_idx = np.zeros(max(int(nnz), 1), dtype=np.int32)
+    lib().oracle_mask_to_index(_p(bm), L, H, nq, nk, _p(row_ptr), _p(col_idx))
+    return row_ptr, col_idx[:nnz]
+
+
+def _strides(a):
+    # element strides of a [B][N][H][d] array whose last dim is contiguous
+    es = a.dtype.itemsize
+    assert a.strides[3] == es, "last dim must be contiguous"
+    return [C.c_int64(a.strides[0] // es), C.c_int64(a.strides[1] // es),
+            C.c_int64(a.strides[2] // es)]
+
+
+def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_threads=0,
+                      return_weight_sum=False):
+    """fp64 block-sparse attention on the exact input bytes.
+
+    Q, K, V: [B][N][H][d] numpy arrays, uint16 (bf16 bits) or uint8 (e4m3 codes; then
+    fp8_scales = (q_scale [B][H][ceil(N/128)], k_scale same, v_scale [B][H][d]) float32).
+    bitmask: uint32 [H][nq][words] (one layer).  items: int array [n][3] of (b, h, qb); default all.
+    Returns out float64 [n_items][128][d] (rows beyond N are 0)  (+ weight sums [n_items][128]).
+    """
+    assert Q.dtype == K.dtype == V.dtype and Q.dtype in (np.uint16, np.uint8)
+    dtype = 0 if Q.dtype == np.uint16 else 1
+    B, N, H, d = Q.shape
+    nq, nk = (N + BQ - 1) // BQ, (N + BK - 1) // BK
+    bm = _c(bitmask, np.uint32)
+    assert bm.shape == (H, nq, (nk + 31) // 32), (bm.shape, (H, nq, (nk + 31) // 32))
+    if items is None:
+        items = np.array([(b, h, qb) for b in range(B) for h in range(H) for qb in range(nq)],
+                         dtype=np.int32)
+    items = np.asarray(items, dtype=np.int32).reshape(-1, 3)
+    ib, ih, iq = (_c(items[:, k], np.int32) for k in range(3))
+    n = items.shape[0]
+    out = np.zeros((n, BQ, d), dtype=np.float64)
+    ws = np.zeros((n, BQ), dtype=np.float64) if return_weight_sum else None
+    if dtype:
+        qs, ks, vs = (_c(x, np.float32) for x in fp8_scales)
+        nsb = (N + 127) // 128
+        assert qs.size == B * H * nsb and ks.size == B * H * nsb and vs.size == B * H * d
+    else:
+        qs = ks = vs = None
+    lib().oracle_block_sparse_attn(
+        _p(Q), _p(K), _p(V), C.c_int(dtype), B, H, N, d,
+        *_strides(Q), *_strides(K), *_strides(V),
+        _p(qs), _p(ks), _p(vs), _p(bm), C.c_double(scale),
+        n, _p(ib), _p(ih), _p(iq), _p(out), _p(ws), C.c_int(n_threads))
+    return (out, ws) if return_weight_sum else out
+
+
+def scatter_items(out_items, items, N, H):
+    """[n_items][128][d] -> dense [B=1][N][H][d] float64 for the covered (h, qb) items."""
+    d = out_items.shape[2]
+    O = np.zeros((1, N, H, d), dtype=np.float64)
+    for t, (b, h, qb) in enumerate(np.asarray(items).reshape(-1, 3)):
+        lo, hi = qb * BQ, min(N, (qb + 1) * BQ)
+        O[b, lo:hi, h, :] = out_items[t, : hi - lo, :]
+    return O
+
+
+def quantize_fp8(Q, K, V):
+    """bf16-bit arrays [B][N][H][d] -> (q8, k8, v8 uint8 packed, q_scale, k_scale, v_scale f32)."""
+    B, N, H, d = Q.shape
+    nsb = (N + 127) // 128
+    q8, k8, v8 = (np.zeros((B, N, H, d), dtype=np.uint8) for _ in range(3))
+    qs = np.zeros((B, H, nsb), dtype=np.float32)
+    ks = np.zeros((B, H, nsb), dtype=np.float32)
+    vs = np.zeros((B, H, d), dtype=np.float32)
+    lib().oracle_quantize_fp8(_p(Q), _p(K), _p(V), B, H, N, d,
+                              *_strides(Q), *_strides(K), *_strides(V),
+                              _p(q8), _p(k8), _p(v8), _p(qs), _p(ks), _p(vs))
+    return q8, k8, v8, qs, ks, vs
+
+
+def e4m3_to_double(code: int) -> float:
+    return float(lib().oracle_e4m3_to_double(int(code)))
+
+
+def float_to_e4m3(x: float) -> int:
+    return int(lib().oracle_float_to_e4m3(float(x)))
+
+
+def retrieve_top1(bank, query, tau):
+    bank = _c(bank, np.float32)
+    query = _c(query, np.float32)
+    n, dim = bank.shape
+    idx, hit, sim = C.c_int32(), C.c_int32(), C.c_double()
+    lib().oracle_retrieve_top1(_p(bank), n, dim, _p(query), C.c_double(tau),
+                               C.byref(idx), C.byref(sim), C.byref(hit))
+    return idx.value, sim.value, bool(hit.value)
+
+
+def visit_refresh(mask, nk, group=8):
+    """mask uint32 [L][H][nq][words]; returns the refreshed copy (PAPER.md:L93 (1))."""
+    m = np.array(mask, dtype=np.uint32, copy=True, order="C")
+    L, H, nq, words = m.shape
+    lib().oracle_visit_refresh(_p(m), L, H, nq, nk, group)
+    return m
