@@ -1,0 +1,184 @@
+/* chorus.h — C ABI of libchorus.so: the B200-native (sm_100a) hot path of Chorus II's
+ * cross-request sparsity reuse (arxiv/paper_2606_25040).
+ *
+ * The path: a new request looks up the most similar historical request; if it is
+ * similar enough, that request's cached block masks "are loaded and used directly by the current
+ * block sparse attention", whose kernels "skip pruned block pairs and evaluate only the retained
+ * ones in QK^T, softmax, and PV".  This library is that path on one GPU:
+ *
+ *   chorus_retrieve_top1          cosine top-1 over stored request embeddings, threshold tau   (L87, L149)
+ *   chorus_visit_refresh          block-pair visit refreshing over groups of layers            (L93 (1), L153)
+ *   chorus_mask_to_index          stored block bitmask  ->  CSR of kept key blocks per query block (L81, L87)
+ *   chorus_quantize_fp8           bf16 Q/K/V -> e4m3 + scales for the FP8 backend              (L97)
+ *   chorus_block_sparse_attn_fwd  block-sparse attention forward, BF16 or FP8 e4m3             (L97)
+ *
+ * Conventions (all entry points)
+ *   - Plain C: pointers and sizes only.  "device" = pointer into CUDA device memory of the current
+ *     device; "host" = ordinary host memory.  Every buffer is owned by the caller; the library
+ *     allocates nothing that outlives a call, keeps no global state, and never frees caller memory.
+ *   - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream)
+ *     and the call returns without synchronising.
+ *   - Errors: an integer status, never an exception.  Argument errors are detected on the host
+ *     before anything is launched.  chorus_last_error() gives a thread-local message.
+ *   - Block geometry is fixed: 128 query rows x 64 keys per block, head_dim 128
+ *     (BASELINE.json north_star; the paper's own run used 64 x 128).
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns
+ *     CHORUS_ERR_CUDA.
+ */
+#ifndef CHORUS_H_
+#define CHORUS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CHORUS_BLOCK_Q 128 /* query rows per mask block */
+#define CHORUS_BLOCK_K 64  /* keys per mask block       */
+#define CHORUS_HEAD_DIM 128
+
+typedef enum {
+    CHORUS_OK = 0,
+    CHORUS_ERR_INVALID_ARG = 1, /* null / misaligned pointer, inconsistent sizes            */
+    CHORUS_ERR_UNSUPPORTED = 2, /* valid request the library does not implement (d != 128)  */
+    CHORUS_ERR_CAPACITY = 3,    /* a size does not fit (nnz > INT32_MAX, workspace too small) */
+    CHORUS_ERR_CUDA = 4         /* a CUDA call failed; see chorus_last_error()              */
+} chorus_status;
+
+typedef enum { CHORUS_BF16 = 0, CHORUS_FP8_E4M3 = 1 } chorus_dtype;
+
+/* ---------------------------------------------------------------------------------------------
+ * Mask decode ("stored, indexed by denoising step, transformer layer, and attention
+ * head"; L87 "loaded and used directly by the current block sparse attention"; L93: the mask is
+ * binary per (head, q-block, k-block)).
+ *
+ * bitmask   device, uint32 [L][H][nq_blk][words], words = ceil(nk_blk / 32), 4-byte aligned.
+ *           Key block kb is bit (kb & 31) (bit 0 = LSB) of word kb >> 5.  Bits >= nk_blk of the
+ *           last word are ignored (they need not be zero).
+ * row_ptr   device, int32 [L*H*nq_blk + 1].  row_ptr[0] = 0; row r = (l*H + h)*nq_blk + qb owns
+ *           col_idx[row_ptr[r] .. row_ptr[r+1]).  Offsets are absolute over the whole mask set.
+ * col_idx   device, int32 [col_cap], kept key-block indices, ascending within each row.
+ *           NULL = count only (row_ptr is still filled).  Entries beyond col_cap are never
+ *           written; the caller sizes col_idx either at an upper bound or from a count-only call
+ *           followed by one 4-byte read of row_ptr[L*H*nq_blk].
+ * workspace device scratch.  Call with workspace == NULL to get the required size in
+ *           *workspace_bytes (nothing is launched); otherwise *workspace_bytes is the size given.
+ * Result is unique (ascending order), so it is compared bit-exactly with the oracle.
+ * Errors: INVALID_ARG (null bitmask/row_ptr/workspace_bytes, L/H/nq_blk/nk_blk <= 0, col_cap < 0),
+ *         CAPACITY (L*H*nq_blk*nk_blk > INT32_MAX, or workspace too small), CUDA.
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                   int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
+                                   void* workspace, size_t* workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Block-pair visit refreshing (PAPER.md:L93 (1); layer_flash = 8 at L153).  Within each group of
+ * `group` consecutive layers a visited map V[h,q,k] records the block pairs activated so far;
+ * "when executing the last layer of the group, any block pair that is still unvisited is forced
+ * into the sparse mask"; the map is reset at the start of the next group.  In place:
+ *     mask[g*group + group-1] |= ~(mask[g*group] | ... | mask[g*group + group-2])
+ * for every complete group g; a trailing partial group is left unchanged.  Pad bits (>= nk_blk)
+ * of the forced layer are left as they were.
+ * bitmask   device, uint32 [L][H][nq_blk][words], updated in place.
+ * Errors: INVALID_ARG (null, sizes <= 0, group < 1), CUDA.
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_visit_refresh(uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                   int group, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Block-sparse attention forward.  For batch b, head h, query i (qb = i / 128):
+ *     J(i)   = { j < N : key block j/64 is in CSR row (h, qb) }        keys >= N are masked
+ *     O[i,:] = sum_{j in J(i)} softmax_j(scale * <Q[i], K[j]>) V[j,:]   softmax over J(i) only
+ * A row with no kept block gives O = 0.  Query rows >= N are not written.
+ *
+ * Shapes/strides: Q, K, V, O are [B][N][H][d]-indexed tensors with arbitrary element strides for
+ * B, N, H (so [B][H][N][d] storage also works); the last dimension (d = 128) is contiguous.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+    int B, H, N, d; /* d must be 128 */
+    int64_t q_stride_b, q_stride_n, q_stride_h; /* in elements */
+    int64_t k_stride_b, k_stride_n, k_stride_h;
+    int64_t v_stride_b, v_stride_n, v_stride_h;
+    int64_t o_stride_b, o_stride_n, o_stride_h;
+} chorus_attn_shape;
+
+/* FP8 scales (device, float).  Dequantised values are code * scale:
+ *   Q^[i,c] = q8[i,c] * q_scale[b][h][i/128]     K^[j,c] = k8[j,c] * k_scale[b][h][j/128]
+ *   V^[j,c] = v8[j,c] * v_scale[b][h][c]
+ * (per-128x128-block Q/K scales, per-channel V scales: BASELINE.json configs[2]). */
+typedef struct {
+    const float* q_scale; /* [B][H][ceil(N/128)] */
+    const float* k_scale; /* [B][H][ceil(N/128)] */
+    const float* v_scale; /* [B][H][d]           */
+} chorus_fp8_scales;
+
+/* Q, K, V   device; dtype BF16: bf16 elements; dtype FP8_E4M3: e4m3 (fn) codes.  Base pointers
+ *           16-byte aligned; strides multiples of 8 (bf16) / 16 (fp8) elements (TMA rules).
+ * row_ptr   device, int32, points at THIS layer's first row: H*nq_blk + 1 readable entries,
+ *           nq_blk = ceil(N/128); the same mask is used for every b.
+ * col_idx   device, the base pointer that row_ptr's absolute offsets index into.  Indices must
+ *           lie in [0, ceil(N/64)) and ascend within a row (what chorus_mask_to_index produces);
+ *           anything else is undefined behaviour.
+ * scale     multiplies QK^T before the softmax (1/sqrt(128) in all workloads).
+ * O         device, bf16 for both dtypes, 16-byte aligned, strides multiples of 8 elements.
+ * fp8       NULL iff dtype == CHORUS_BF16.
+ * Accuracy against the fp64 oracle on the same input bytes (BASELINE.json north_star):
+ *           BF16: max|err| <= 2e-2, mean|err| <= 2e-3;  FP8: max|err| <= 8e-2, cosine >= 0.995.
+ * Errors: INVALID_ARG (null pointer, misalignment, bad strides, N/H/B <= 0, fp8/dtype mismatch),
+ *         UNSUPPORTED (d != 128, unknown dtype), CUDA.
+ */
+chorus_status chorus_block_sparse_attn_fwd(const void* Q, const void* K, const void* V,
+                                           const int32_t* row_ptr, const int32_t* col_idx,
+                                           float scale, chorus_dtype dtype, void* O,
+                                           const chorus_attn_shape* shape,
+                                           const chorus_fp8_scales* fp8, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * FP8 quantisation pre-pass for dtype = CHORUS_FP8_E4M3 (PAPER.md:L97 says only "FP8
+ * quantization"; granularity and formula are BASELINE.json configs[2] / DESIGN.md R10-R11):
+ *     s  = max(amax, 1e-12) / 448      x8 = e4m3_rne_saturate(x / s)       (fp32 arithmetic)
+ * with amax over one (b, h, 128-token block) for Q and K, and over all tokens of one
+ * (b, h, channel) for V; only tokens < N count.
+ * Q, K, V   device, bf16, [B][N][H][d] with the strides in `shape` (o_stride_* ignored).
+ * q8,k8,v8  device, uint8 e4m3 codes, PACKED [B][N][H][d] (stride_n = H*d, stride_h = d).
+ * q_scale, k_scale  device float [B][H][ceil(N/128)];  v_scale  device float [B][H][d].
+ * Errors: INVALID_ARG, UNSUPPORTED (d != 128), CUDA.
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_quantize_fp8(const void* Q, const void* K, const void* V,
+                                  const chorus_attn_shape* shape, void* q8, void* k8, void* v8,
+                                  float* q_scale, float* k_scale, float* v_scale,
+                                  void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Retrieval ("k-nearest-neighbor search under cosine similarity over the joint text
+ * and image embeddings; if the similarity to the top neighbor exceeds a threshold tau, its cached
+ * sparse masks are loaded"; tau = 0.4 at L149).  Embeddings are unit-norm, so cosine = dot.
+ * bank      device, float [n][dim], row-major, 16-byte aligned, dim % 4 == 0.
+ * query     device, float [dim].
+ * best_idx  device int32: argmax_j <bank[j], query>, ties -> lowest j.
+ * best_sim  device float: that dot product (fp32 accumulation).
+ * hit       device int32: 1 if best_sim >= tau else 0 (0 => caller falls back, L87/L149).
+ * workspace device scratch, same query protocol as chorus_mask_to_index.
+ * Errors: INVALID_ARG, CAPACITY (workspace too small), CUDA.
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_retrieve_top1(const float* bank, int n, int dim, const float* query, float tau,
+                                   int32_t* best_idx, float* best_sim, int32_t* hit,
+                                   void* workspace, size_t* workspace_bytes, void* cuda_stream);
+
+/* Thread-local description of the last error returned on this thread ("" if none). */
+const char* chorus_last_error(void);
+
+/* Library/ABI version and build info, static storage. */
+const char* chorus_version(void);
+
+/* Number of kernel launches enqueued by this library on the calling thread since the last
+ * chorus_reset_launch_count() (bench.py reports it as gpu_launches). */
+int64_t chorus_launch_count(void);
+void chorus_reset_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHORUS_H_ */

@@ -2,7 +2,7 @@
 
     python -m oracle.build
 
-g++ -O3 -march=native -fopenmp; no CUDA, no code from paper_2606_25040_b200/.
+g++ -O3 -march=native -fopenmp; no CUDA and nothing taken from the CUDA package.
 """
 from __future__ import annotations
 

@@ -1,0 +1,210 @@
+"""ctypes binding over libchorus.so — same names as include/chorus.h, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; torch is used for device memory and the
+current stream.  There is no CPU fallback: if the library is missing or a call fails, a
+ChorusError is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libchorus.so")
+
+CHORUS_OK, CHORUS_ERR_INVALID_ARG, CHORUS_ERR_UNSUPPORTED, CHORUS_ERR_CAPACITY, CHORUS_ERR_CUDA = range(5)
+CHORUS_BF16, CHORUS_FP8_E4M3 = 0, 1
+BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
+
+EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
+           "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_last_error", "chorus_version",
+           "chorus_launch_count", "chorus_reset_launch_count"]
+
+
+class ChorusError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libchorus status {status}: {msg}")
+        self.status = status
+
+
+class AttnShape(C.Structure):
+    _fields_ = [("B", C.c_int), ("H", C.c_int), ("N", C.c_int), ("d", C.c_int)] + [
+        (f"{t}_stride_{a}", C.c_int64) for t in "qkvo" for a in "bnh"]
+
+
+class Fp8Scales(C.Structure):
+    _fields_ = [("q_scale", C.c_void_p), ("k_scale", C.c_void_p), ("v_scale", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libchorus.so (built in-tree by `python -m paper_2606_25040_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ChorusError(CHORUS_ERR_CUDA, f"{LIB_PATH} not found: build it with "
+                              "`python -m paper_2606_25040_b200.build` (there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.chorus_last_error.restype = C.c_char_p
+        L.chorus_version.restype = C.c_char_p
+        L.chorus_launch_count.restype = C.c_int64
+        L.chorus_mask_to_index.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p,
+                                           C.c_void_p, C.c_int64, C.c_void_p,
+                                           C.POINTER(C.c_size_t), C.c_void_p]
+        L.chorus_visit_refresh.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                           C.c_void_p]
+        L.chorus_block_sparse_attn_fwd.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                                   C.c_void_p, C.c_float, C.c_int, C.c_void_p,
+                                                   C.POINTER(AttnShape), C.POINTER(Fp8Scales),
+                                                   C.c_void_p]
+        L.chorus_quantize_fp8.argtypes = [C.c_void_p] * 3 + [C.POINTER(AttnShape)] + [C.c_void_p] * 7
+        L.chorus_retrieve_top1.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_float,
+                                           C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                           C.POINTER(C.c_size_t), C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _check(status: int):
+    if status != CHORUS_OK:
+        raise ChorusError(status, lib().chorus_last_error().decode())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _ptr(t):
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def chorus_version() -> str:
+    return lib().chorus_version().decode()
+
+
+def chorus_launch_count() -> int:
+    return int(lib().chorus_launch_count())
+
+
+def chorus_reset_launch_count() -> None:
+    lib().chorus_reset_launch_count()
+
+
+def mask_to_index_workspace_bytes(L: int, H: int, nq_blk: int, nk_blk: int) -> int:
+    n = C.c_size_t(0)
+    _check(lib().chorus_mask_to_index(None, L, H, nq_blk, nk_blk, None, None, 0, None, C.byref(n), None))
+    return int(n.value)
+
+
+def chorus_mask_to_index(bitmask, nk_blk: int, row_ptr=None, col_idx=None, workspace=None,
+                         stream=None, count_only=False):
+    """bitmask: cuda int32/uint32-bits tensor [L][H][nq][words].  Returns (row_ptr, col_idx).
+
+    If col_idx is not given: count-only pass, one 4-byte read of nnz, allocation, second pass
+    (the protocol include/chorus.h describes)."""
+    L, H, nq, words = bitmask.shape
+    assert bitmask.is_cuda and bitmask.is_contiguous() and bitmask.element_size() == 4
+    assert words == (nk_blk + 31) // 32
+    rows = L * H * nq
+    dev = bitmask.device
+    if row_ptr is None:
+        row_ptr = torch.empty(rows + 1, dtype=torch.int32, device=dev)
+    if workspace is None:
+        workspace = torch.empty(max(mask_to_index_workspace_bytes(L, H, nq, nk_blk), 4),
+                                dtype=torch.uint8, device=dev)
+    wsb = C.c_size_t(workspace.numel())
+    if col_idx is None:
+        _check(lib().chorus_mask_to_index(_ptr(bitmask), L, H, nq, nk_blk, _ptr(row_ptr), None, 0,
+                                          _ptr(workspace), C.byref(wsb), _stream(stream)))
+        if count_only:
+            return row_ptr, None
+        nnz = int(row_ptr[-1].item())
+        col_idx = torch.empty(max(nnz, 1), dtype=torch.int32, device=dev)
+    _check(lib().chorus_mask_to_index(_ptr(bitmask), L, H, nq, nk_blk, _ptr(row_ptr), _ptr(col_idx),
+                                      col_idx.numel(), _ptr(workspace), C.byref(wsb), _stream(stream)))
+    return row_ptr, col_idx
+
+
+def chorus_visit_refresh(bitmask, nk_blk: int, group: int = 8, stream=None):
+    L, H, nq, words = bitmask.shape
+    assert bitmask.is_cuda and bitmask.is_contiguous() and bitmask.element_size() == 4
+    _check(lib().chorus_visit_refresh(_ptr(bitmask), L, H, nq, nk_blk, group, _stream(stream)))
+    return bitmask
+
+
+def attn_shape(Q, K, V, O=None) -> AttnShape:
+    B, N, H, d = Q.shape
+    s = AttnShape(B=B, H=H, N=N, d=d)
+    for name, t in (("q", Q), ("k", K), ("v", V), ("o", O)):
+        if t is None:
+            continue
+        assert t.stride(3) == 1, "last dimension must be contiguous"
+        setattr(s, f"{name}_stride_b", t.stride(0))
+        setattr(s, f"{name}_stride_n", t.stride(1))
+        setattr(s, f"{name}_stride_h", t.stride(2))
+    return s
+
+
+def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype: int = CHORUS_BF16,
+                                 O=None, fp8_scales=None, stream=None):
+    """Q, K, V: cuda tensors indexed [B][N][H][d] (bf16, or uint8/float8_e4m3fn codes for FP8).
+    row_ptr: this layer's H*nq+1 entries (a view into the full row_ptr is fine).  Returns O (bf16)."""
+    assert Q.is_cuda and K.is_cuda and V.is_cuda
+    B, N, H, d = Q.shape
+    if O is None:
+        O = torch.empty((B, N, H, d), dtype=torch.bfloat16, device=Q.device)
+    shape = attn_shape(Q, K, V, O)
+    sc = None
+    if fp8_scales is not None:
+        sc = Fp8Scales(*(x.data_ptr() for x in fp8_scales))
+    _check(lib().chorus_block_sparse_attn_fwd(_ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx),
+                                              C.c_float(scale), dtype, _ptr(O), C.byref(shape),
+                                              C.byref(sc) if sc is not None else None,
+                                              _stream(stream)))
+    return O
+
+
+def chorus_quantize_fp8(Q, K, V, out=None, stream=None):
+    """bf16 Q/K/V [B][N][H][d] -> (q8, k8, v8 uint8 packed, q_scale, k_scale, v_scale)."""
+    B, N, H, d = Q.shape
+    dev = Q.device
+    nsb = (N + 127) // 128
+    if out is None:
+        out = tuple(torch.empty((B, N, H, d), dtype=torch.uint8, device=dev) for _ in range(3)) + (
+            torch.empty((B, H, nsb), dtype=torch.float32, device=dev),
+            torch.empty((B, H, nsb), dtype=torch.float32, device=dev),
+            torch.empty((B, H, d), dtype=torch.float32, device=dev))
+    shape = attn_shape(Q, K, V)
+    _check(lib().chorus_quantize_fp8(_ptr(Q), _ptr(K), _ptr(V), C.byref(shape), *(_ptr(t) for t in out),
+                                     _stream(stream)))
+    return out
+
+
+def retrieve_workspace_bytes(n: int, dim: int) -> int:
+    b = C.c_size_t(0)
+    _check(lib().chorus_retrieve_top1(None, n, dim, None, C.c_float(0), None, None, None, None,
+                                      C.byref(b), None))
+    return int(b.value)
+
+
+def chorus_retrieve_top1(bank, query, tau: float, out=None, workspace=None, stream=None):
+    """bank float32 [n][dim], query float32 [dim] (cuda).  Returns device tensors
+    (best_idx int32[1], best_sim float32[1], hit int32[1]); nothing is synchronised."""
+    n, dim = bank.shape
+    dev = bank.device
+    if out is None:
+        out = (torch.empty(1, dtype=torch.int32, device=dev),
+               torch.empty(1, dtype=torch.float32, device=dev),
+               torch.empty(1, dtype=torch.int32, device=dev))
+    if workspace is None:
+        workspace = torch.empty(retrieve_workspace_bytes(n, dim), dtype=torch.uint8, device=dev)
+    wsb = C.c_size_t(workspace.numel())
+    _check(lib().chorus_retrieve_top1(_ptr(bank), n, dim, _ptr(query), C.c_float(tau), _ptr(out[0]),
+                                      _ptr(out[1]), _ptr(out[2]), _ptr(workspace), C.byref(wsb),
+                                      _stream(stream)))
+    return out

@@ -1,0 +1,260 @@
+// chorus_api.cu — the C ABI of libchorus.so (include/chorus.h): argument validation, TMA tensor-map
+// construction and kernel launches.  No torch types, no allocation, no synchronisation.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "chorus_internal.h"
+
+namespace chorus {
+namespace {
+
+thread_local char g_err[512] = "";
+thread_local int64_t g_launches = 0;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (fn) return fn;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+        return nullptr;
+    fn = reinterpret_cast<EncodeTiledFn>(p);
+    return fn;
+}
+
+// Tensor map over a [B][N][H][d]-indexed tensor with element strides (d contiguous):
+// dims (innermost first) = {d, N, H, B}; box = {box_cols, box_rows, 1, 1}; 128-byte swizzle.
+chorus_status make_tmap(CUtensorMap* tm, const void* base, int elem_bytes, int B, int H, int N,
+                        int d, int64_t sb, int64_t sn, int64_t sh, int box_cols, int box_rows,
+                        const char* name) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return set_error(CHORUS_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    const CUtensorMapDataType dt =
+        elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8;
+    cuuint64_t dims[4] = {static_cast<cuuint64_t>(d), static_cast<cuuint64_t>(N),
+                          static_cast<cuuint64_t>(H), static_cast<cuuint64_t>(B)};
+    // a size-1 dimension never advances; give it a harmless, valid stride
+    const int64_t row = static_cast<int64_t>(d);
+    if (N == 1) sn = row;
+    if (H == 1) sh = row;
+    if (B == 1) sb = row;
+    cuuint64_t strides[3] = {static_cast<cuuint64_t>(sn) * elem_bytes,
+                             static_cast<cuuint64_t>(sh) * elem_bytes,
+                             static_cast<cuuint64_t>(sb) * elem_bytes};
+    cuuint32_t box[4] = {static_cast<cuuint32_t>(box_cols), static_cast<cuuint32_t>(box_rows), 1, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = enc(tm, dt, 4, const_cast<void*>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS)
+        return set_error(CHORUS_ERR_CUDA, "cuTensorMapEncodeTiled(%s) failed with CUresult %d", name,
+                         static_cast<int>(r));
+    return CHORUS_OK;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace
+
+chorus_status set_error(chorus_status st, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+chorus_status check_cuda(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return CHORUS_OK;
+    return set_error(CHORUS_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+void count_launch(int n) { g_launches += n; }
+
+}  // namespace chorus
+
+using namespace chorus;
+
+extern "C" {
+
+const char* chorus_last_error(void) { return g_err; }
+
+const char* chorus_version(void) {
+    return "libchorus 0.1 (sm_100a; blocks 128q x 64k, head_dim 128; built " __DATE__ ")";
+}
+
+int64_t chorus_launch_count(void) { return g_launches; }
+void chorus_reset_launch_count(void) { g_launches = 0; }
+
+chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                   int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
+                                   void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!workspace_bytes) return set_error(CHORUS_ERR_INVALID_ARG, "workspace_bytes is null");
+    if (L <= 0 || H <= 0 || nq_blk <= 0 || nk_blk <= 0)
+        return set_error(CHORUS_ERR_INVALID_ARG, "L, H, nq_blk, nk_blk must be positive (%d %d %d %d)",
+                         L, H, nq_blk, nk_blk);
+    const int64_t rows = static_cast<int64_t>(L) * H * nq_blk;
+    if (rows * nk_blk > INT32_MAX)
+        return set_error(CHORUS_ERR_CAPACITY, "L*H*nq_blk*nk_blk = %lld exceeds INT32_MAX",
+                         static_cast<long long>(rows * nk_blk));
+    const size_t need = decode_workspace_bytes(rows);
+    if (!workspace) {
+        *workspace_bytes = need;
+        return CHORUS_OK;
+    }
+    if (!bitmask || !row_ptr) return set_error(CHORUS_ERR_INVALID_ARG, "bitmask / row_ptr is null");
+    if (col_cap < 0) return set_error(CHORUS_ERR_INVALID_ARG, "col_cap < 0");
+    if ((reinterpret_cast<uintptr_t>(bitmask) | reinterpret_cast<uintptr_t>(row_ptr) |
+         reinterpret_cast<uintptr_t>(col_idx) | reinterpret_cast<uintptr_t>(workspace)) & 3u)
+        return set_error(CHORUS_ERR_INVALID_ARG, "pointers must be 4-byte aligned");
+    if (*workspace_bytes < need)
+        return set_error(CHORUS_ERR_CAPACITY, "workspace too small: %zu < %zu", *workspace_bytes, need);
+    const int words = (nk_blk + 31) / 32;
+    return check_cuda(launch_mask_decode(bitmask, rows, nk_blk, words, row_ptr, col_idx, col_cap,
+                                         workspace, static_cast<cudaStream_t>(cuda_stream)),
+                      "mask decode launch");
+}
+
+chorus_status chorus_visit_refresh(uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                   int group, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!bitmask) return set_error(CHORUS_ERR_INVALID_ARG, "bitmask is null");
+    if (L <= 0 || H <= 0 || nq_blk <= 0 || nk_blk <= 0 || group < 1)
+        return set_error(CHORUS_ERR_INVALID_ARG, "L, H, nq_blk, nk_blk must be positive, group >= 1");
+    const int words = (nk_blk + 31) / 32;
+    return check_cuda(launch_visit_refresh(bitmask, L, static_cast<int64_t>(H) * nq_blk * words,
+                                           words, nk_blk, group,
+                                           static_cast<cudaStream_t>(cuda_stream)),
+                      "visit refresh launch");
+}
+
+static chorus_status validate_shape(const chorus_attn_shape* s, int elem_mult, bool check_o) {
+    if (!s) return set_error(CHORUS_ERR_INVALID_ARG, "shape is null");
+    if (s->d != CHORUS_HEAD_DIM)
+        return set_error(CHORUS_ERR_UNSUPPORTED, "head_dim %d is not supported (only 128)", s->d);
+    if (s->B <= 0 || s->H <= 0 || s->N <= 0)
+        return set_error(CHORUS_ERR_INVALID_ARG, "B, H, N must be positive (%d %d %d)", s->B, s->H, s->N);
+    const int64_t st[9] = {s->q_stride_b, s->q_stride_n, s->q_stride_h, s->k_stride_b, s->k_stride_n,
+                           s->k_stride_h, s->v_stride_b, s->v_stride_n, s->v_stride_h};
+    const int dimsz[3] = {s->B, s->N, s->H};
+    for (int i = 0; i < 9; ++i) {
+        if (dimsz[i % 3] == 1) continue;
+        if (st[i] <= 0 || st[i] % elem_mult)
+            return set_error(CHORUS_ERR_INVALID_ARG,
+                             "Q/K/V stride #%d = %lld must be a positive multiple of %d elements", i,
+                             static_cast<long long>(st[i]), elem_mult);
+    }
+    if (check_o) {
+        const int64_t so[3] = {s->o_stride_b, s->o_stride_n, s->o_stride_h};
+        for (int i = 0; i < 3; ++i) {
+            if (dimsz[i] == 1) continue;
+            if (so[i] <= 0 || so[i] % 8)
+                return set_error(CHORUS_ERR_INVALID_ARG,
+                                 "O stride #%d = %lld must be a positive multiple of 8 elements", i,
+                                 static_cast<long long>(so[i]));
+        }
+    }
+    return CHORUS_OK;
+}
+
+chorus_status chorus_block_sparse_attn_fwd(const void* Q, const void* K, const void* V,
+                                           const int32_t* row_ptr, const int32_t* col_idx,
+                                           float scale, chorus_dtype dtype, void* O,
+                                           const chorus_attn_shape* shape,
+                                           const chorus_fp8_scales* fp8, void* cuda_stream) {
+    g_err[0] = 0;
+    if (dtype != CHORUS_BF16 && dtype != CHORUS_FP8_E4M3)
+        return set_error(CHORUS_ERR_UNSUPPORTED, "unknown dtype %d", static_cast<int>(dtype));
+    if (!Q || !K || !V || !O || !row_ptr || !col_idx)
+        return set_error(CHORUS_ERR_INVALID_ARG, "Q, K, V, O, row_ptr, col_idx must be non-null");
+    if (!aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
+        return set_error(CHORUS_ERR_INVALID_ARG, "Q, K, V, O must be 16-byte aligned");
+    if ((dtype == CHORUS_FP8_E4M3) != (fp8 != nullptr))
+        return set_error(CHORUS_ERR_INVALID_ARG, "fp8 scales must be given iff dtype is FP8_E4M3");
+    if (fp8 && (!fp8->q_scale || !fp8->k_scale || !fp8->v_scale))
+        return set_error(CHORUS_ERR_INVALID_ARG, "fp8 scale pointers must be non-null");
+    const int eb = dtype == CHORUS_BF16 ? 2 : 1;
+    chorus_status st = validate_shape(shape, 16 / eb, true);
+    if (st != CHORUS_OK) return st;
+    const chorus_attn_shape& s = *shape;
+
+    CUtensorMap tmQ, tmK, tmV, tmO;
+    const int cols = 128 / eb;  // 128-byte inner box: 64 bf16 or 128 fp8 channels
+    if ((st = make_tmap(&tmQ, Q, eb, s.B, s.H, s.N, s.d, s.q_stride_b, s.q_stride_n, s.q_stride_h,
+                        cols, CHORUS_BLOCK_Q, "Q")) != CHORUS_OK) return st;
+    if ((st = make_tmap(&tmK, K, eb, s.B, s.H, s.N, s.d, s.k_stride_b, s.k_stride_n, s.k_stride_h,
+                        cols, CHORUS_BLOCK_K, "K")) != CHORUS_OK) return st;
+    if ((st = make_tmap(&tmV, V, eb, s.B, s.H, s.N, s.d, s.v_stride_b, s.v_stride_n, s.v_stride_h,
+                        cols, CHORUS_BLOCK_K, "V")) != CHORUS_OK) return st;
+    if ((st = make_tmap(&tmO, O, 2, s.B, s.H, s.N, s.d, s.o_stride_b, s.o_stride_n, s.o_stride_h,
+                        64, 32, "O")) != CHORUS_OK) return st;
+
+    AttnParams p;
+    p.row_ptr = row_ptr;
+    p.col_idx = col_idx;
+    p.O = O;
+    p.o_sb = s.o_stride_b; p.o_sn = s.o_stride_n; p.o_sh = s.o_stride_h;
+    p.B = s.B; p.H = s.H; p.N = s.N;
+    p.nq = (s.N + CHORUS_BLOCK_Q - 1) / CHORUS_BLOCK_Q;
+    p.nk = (s.N + CHORUS_BLOCK_K - 1) / CHORUS_BLOCK_K;
+    p.scale_log2 = scale * 1.4426950408889634f;
+    p.q_scale = fp8 ? fp8->q_scale : nullptr;
+    p.k_scale = fp8 ? fp8->k_scale : nullptr;
+    p.v_scale = fp8 ? fp8->v_scale : nullptr;
+    cudaError_t e = launch_attn_fwd(tmQ, tmK, tmV, tmO, p, dtype, static_cast<cudaStream_t>(cuda_stream));
+    if (e == cudaErrorNotSupported)
+        return set_error(CHORUS_ERR_UNSUPPORTED, "dtype %d not implemented by this build", (int)dtype);
+    return check_cuda(e, "attention launch");
+}
+
+chorus_status chorus_quantize_fp8(const void* Q, const void* K, const void* V,
+                                  const chorus_attn_shape* shape, void* q8, void* k8, void* v8,
+                                  float* q_scale, float* k_scale, float* v_scale,
+                                  void* cuda_stream) {
+    g_err[0] = 0;
+    if (!Q || !K || !V || !q8 || !k8 || !v8 || !q_scale || !k_scale || !v_scale)
+        return set_error(CHORUS_ERR_INVALID_ARG, "all pointers must be non-null");
+    if (!aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(q8) || !aligned16(k8) ||
+        !aligned16(v8))
+        return set_error(CHORUS_ERR_INVALID_ARG, "tensors must be 16-byte aligned");
+    chorus_status st = validate_shape(shape, 8, false);
+    if (st != CHORUS_OK) return st;
+    return check_cuda(launch_quantize_fp8(Q, K, V, *shape, q8, k8, v8, q_scale, k_scale, v_scale,
+                                          static_cast<cudaStream_t>(cuda_stream)),
+                      "fp8 quantise launch");
+}
+
+chorus_status chorus_retrieve_top1(const float* bank, int n, int dim, const float* query, float tau,
+                                   int32_t* best_idx, float* best_sim, int32_t* hit,
+                                   void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!workspace_bytes) return set_error(CHORUS_ERR_INVALID_ARG, "workspace_bytes is null");
+    if (n <= 0 || dim <= 0 || (dim & 3))
+        return set_error(CHORUS_ERR_INVALID_ARG, "n > 0, dim > 0 and dim %% 4 == 0 required (%d, %d)", n, dim);
+    const size_t need = retrieve_workspace_bytes(n);
+    if (!workspace) {
+        *workspace_bytes = need;
+        return CHORUS_OK;
+    }
+    if (!bank || !query || !best_idx || !best_sim || !hit)
+        return set_error(CHORUS_ERR_INVALID_ARG, "bank, query, best_idx, best_sim, hit must be non-null");
+    if (!aligned16(bank) || !aligned16(query))
+        return set_error(CHORUS_ERR_INVALID_ARG, "bank and query must be 16-byte aligned");
+    if (*workspace_bytes < need)
+        return set_error(CHORUS_ERR_CAPACITY, "workspace too small: %zu < %zu", *workspace_bytes, need);
+    if (static_cast<size_t>(dim) * sizeof(float) > 200 * 1024)
+        return set_error(CHORUS_ERR_CAPACITY, "dim %d does not fit the shared-memory query buffer", dim);
+    return check_cuda(launch_retrieve_top1(bank, n, dim, query, tau, best_idx, best_sim, hit,
+                                           workspace, static_cast<cudaStream_t>(cuda_stream)),
+                      "retrieve launch");
+}
+
+}  // extern "C"

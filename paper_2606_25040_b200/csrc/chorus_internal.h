@@ -1,0 +1,52 @@
+// chorus_internal.h — declarations shared by the translation units of libchorus.so (host side).
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "../../include/chorus.h"
+
+namespace chorus {
+
+// thread-local error string + launch counter (chorus_api.cu)
+chorus_status set_error(chorus_status st, const char* fmt, ...);
+chorus_status check_cuda(cudaError_t e, const char* what);
+void count_launch(int n = 1);
+
+// ---- mask_decode.cu ----------------------------------------------------------------------------
+size_t decode_workspace_bytes(int64_t rows);
+cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, int words,
+                               int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
+                               cudaStream_t stream);
+cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_layer, int words,
+                                 int nk, int group, cudaStream_t stream);
+
+// ---- retrieve.cu -------------------------------------------------------------------------------
+size_t retrieve_workspace_bytes(int n);
+cudaError_t launch_retrieve_top1(const float* bank, int n, int dim, const float* query, float tau,
+                                 int32_t* best_idx, float* best_sim, int32_t* hit, void* workspace,
+                                 cudaStream_t stream);
+
+// ---- quantize_fp8.cu ---------------------------------------------------------------------------
+cudaError_t launch_quantize_fp8(const void* Q, const void* K, const void* V,
+                                const chorus_attn_shape& s, void* q8, void* k8, void* v8,
+                                float* q_scale, float* k_scale, float* v_scale,
+                                cudaStream_t stream);
+
+// ---- attn_fwd.cu -------------------------------------------------------------------------------
+struct AttnParams {
+    const int32_t* row_ptr;
+    const int32_t* col_idx;
+    void* O;
+    int64_t o_sb, o_sn, o_sh;
+    int B, H, N, nq, nk;
+    float scale_log2;  // scale * log2(e)
+    const float* q_scale;
+    const float* k_scale;
+    const float* v_scale;
+};
+cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
+                            const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
+                            cudaStream_t stream);
+
+}  // namespace chorus

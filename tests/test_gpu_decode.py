@@ -1,0 +1,81 @@
+"""GPU parity: chorus_mask_to_index / chorus_visit_refresh vs the oracle, bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from gpu_common import dev, dmask
+from paper_2606_25040_b200 import binding as B
+from paper_2606_25040_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def check(bm, nk):
+    rp_o, ci_o = oracle.mask_to_index(bm, nk)
+    rp, ci = B.chorus_mask_to_index(dmask(bm), nk)
+    torch.cuda.synchronize()
+    assert np.array_equal(rp.cpu().numpy(), rp_o)
+    assert np.array_equal(ci.cpu().numpy()[: len(ci_o)], ci_o)
+    return rp, ci
+
+
+@pytest.mark.parametrize("L,H,nq,nk,rho", [
+    (1, 2, 32, 64, 0.5), (2, 3, 7, 33, 0.3), (1, 2, 5, 1182, 0.15), (3, 2, 9, 512, 0.25),
+    (1, 1, 1, 1, 1.0), (2, 2, 130, 31, 0.5), (1, 1, 300, 32, 0.02), (1, 3, 129, 1025, 0.1)])
+def test_random_masks_with_garbage_pad_bits(L, H, nq, nk, rho):
+    g = np.random.default_rng(nk * 7 + nq)
+    bm = W.pack_bits(g.random((L, H, nq, nk)) < rho)
+    if nk % 32:
+        bm[..., -1] |= np.uint32((0xFFFFFFFF << (nk % 32)) & 0xFFFFFFFF)
+    check(bm, nk)
+
+
+def test_adversarial_rows():
+    nk, nq = 100, 260
+    keep = np.zeros((1, 1, nq, nk), bool)
+    keep[0, 0, 1] = True                 # full row
+    keep[0, 0, 2, 99] = True             # single bit in the last (partial) word
+    keep[0, 0, 3, 0] = True
+    keep[0, 0, 127:130, ::3] = True      # rows straddling a 128-row block boundary
+    keep[0, 0, 259, 31:34] = True
+    check(W.pack_bits(keep), nk)
+    check(np.zeros((1, 2, 5, 4), np.uint32), nk)           # empty mask: all row_ptr = 0
+    check(np.full((1, 2, 5, 4), 0xFFFFFFFF, np.uint32), nk)  # full mask with garbage pad bits
+
+
+def test_full_size_layer_masks_cfg2_cfg4():
+    for cfg in (W.CFG2, W.CFG4):
+        bm = W.layer_mask(cfg)[None]
+        rp, ci = check(bm, cfg.nk)
+        per_row = 128 if cfg is W.CFG2 else 177
+        assert int(rp[-1].item()) == cfg.H * cfg.nq * per_row
+
+
+def test_multi_layer_mask_set_and_count_only_and_capacity():
+    cfg = W.scaled(W.CFG2, H=4)
+    bm = np.stack([W.layer_mask(cfg, seed=77 + 100 * l, density=0.1 + 0.1 * l) for l in range(3)])
+    rp_o, ci_o = oracle.mask_to_index(bm, cfg.nk)
+    d = dmask(bm)
+    rp, none = B.chorus_mask_to_index(d, cfg.nk, count_only=True)
+    torch.cuda.synchronize()
+    assert none is None and np.array_equal(rp.cpu().numpy(), rp_o)
+    # col_cap smaller than nnz: nothing beyond col_cap is written
+    cap = len(ci_o) // 2
+    buf = torch.full((len(ci_o),), -7, dtype=torch.int32, device=dev())
+    B.chorus_mask_to_index(d, cfg.nk, col_idx=buf[:cap])
+    torch.cuda.synchronize()
+    got = buf.cpu().numpy()
+    assert np.array_equal(got[:cap], ci_o[:cap]) and np.all(got[cap:] == -7)
+
+
+def test_visit_refresh_matches_oracle():
+    nk, nq, H, L = 45, 3, 2, 19
+    g = np.random.default_rng(3)
+    bm = W.pack_bits(g.random((L, H, nq, nk)) < 0.2)
+    bm[..., -1] |= np.uint32(0xFFFFE000)          # garbage pad bits must be left as they are
+    ref = oracle.visit_refresh(bm, nk, group=8)
+    d = dmask(bm)
+    B.chorus_visit_refresh(d, nk, group=8)
+    torch.cuda.synchronize()
+    assert np.array_equal(d.cpu().numpy().view(np.uint32), ref)
