@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of the Chorus II sparsity-reuse hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl chorus|reference] [--workload cfg2|cfg1|cfg4]
+
+One "step" = one pass of the hot path over one attention layer's inputs (BASELINE.json configs[1]:
+480p Wan-2.2-14B-shaped layer, H=40, N=32760, d=128, 25 % density block masks):
+    chorus_mask_to_index (stored bitmask -> CSR)  ->  chorus_block_sparse_attn_fwd (BF16)
+    -> chorus_quantize_fp8 -> chorus_block_sparse_attn_fwd (FP8)         [FP8 leg when the build has it]
+Metric: effective TFLOP/s on kept tiles, FLOPs = 4*N^2*d*H*density per attention call
+(BASELINE.json north_star).  Prints ONE JSON line (rank 0).
+
+Multi-GPU (torchrun): the path has no exchange step (one GPU per attention call, north_star), so
+N ranks run N independent replicas ("replicas only"); `value` is the aggregate.
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the
+same workload on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "block-sparse attn effective TFLOPS (kept tiles) @480p"
+UNIT = "TFLOP/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16": d["bf16_tflops"],
+                "bf16_sustained": d.get("bf16_tflops_sustained"), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+
+
+def get_cfg(name):
+    from paper_2606_25040_b200 import workloads as W
+    return {"cfg1": W.CFG1, "cfg2": W.CFG2, "cfg4": W.CFG4}[name]
+
+
+def attn_flops(cfg, density):
+    return 4.0 * cfg.N * cfg.N * cfg.d * cfg.H * density
+
+
+# --------------------------------------------------------------------------------------------------
+# clock sampling during the timed region
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.samples = []
+        self._stop = threading.Event()
+        self._thr = None
+
+    def _sample_once(self):
+        try:
+            out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}",
+                                  "--format=csv,noheader,nounits"], capture_output=True, text=True,
+                                 timeout=5).stdout.strip().splitlines()
+            if out:
+                f = [x.strip() for x in out[0].split(",")]
+                self.samples.append((float(f[0]), float(f[1]), f[3:]))
+        except Exception:
+            pass
+
+    def _run(self):
+        while not self._stop.is_set():
+            self._sample_once()
+            self._stop.wait(0.1)
+
+    def start(self):
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join(timeout=10)
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for _, _, fl in self.samples for n, v in zip(names, fl) if v.lower().startswith("active")})
+        return {"sm_mhz": statistics.median(s[0] for s in self.samples),
+                "sm_max_mhz": self.samples[0][1], "reasons": reasons, "samples": len(self.samples)}
+
+
+# --------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline / --impl reference)
+# --------------------------------------------------------------------------------------------------
+def oracle_sample_time(cfg, Qb, Kb, Vb, bm, n_items, seed=0):
+    """Time the oracle, as it stands, on n_items (head, q-block) items of the workload."""
+    import oracle
+    g = np.random.default_rng(seed)
+    items = np.stack([np.zeros(n_items, np.int64), g.integers(0, Qb.shape[2], n_items),
+                      g.integers(0, cfg.nq, n_items)], axis=1).astype(np.int32)
+    keep_rows = 0
+    from paper_2606_25040_b200 import workloads as W
+    keep = W.unpack_bits(bm, cfg.nk)
+    valid = np.minimum(64, cfg.N - 64 * np.arange(cfg.nk))
+    flops = 0.0
+    for _, h, qb in items:
+        rows = min(128, cfg.N - 128 * qb)
+        keys = float(valid[keep[h, qb]].sum())
+        flops += 4.0 * rows * keys * cfg.d
+        keep_rows += rows
+    t0 = time.perf_counter()
+    oracle.block_sparse_attn(Qb, Kb, Vb, bm, cfg.scale, items=items)
+    dt = time.perf_counter() - t0
+    return dt, flops, oracle.num_threads()
+
+
+def cpu_baseline(cfg, Qb, Kb, Vb, bm, budget_s=15.0):
+    import oracle
+    cores = oracle.num_threads()
+    dt, fl, _ = oracle_sample_time(cfg, Qb, Kb, Vb, bm, cores)          # probe: one item per core
+    n = int(max(cores, min(64 * cores, cores * round(budget_s / max(dt, 1e-3)))))
+    dt, fl, _ = oracle_sample_time(cfg, Qb, Kb, Vb, bm, n, seed=1)
+    return {"value": fl / dt / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n} random (head, 128-row query block) items of {cfg.name} "
+                      f"(of {Qb.shape[2] * cfg.nq}), fp64, {dt:.1f} s",
+            "seconds": dt}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2606_25040_b200 import workloads as W
+    import oracle
+    cfg = get_cfg(args.workload)
+    heads = min(cfg.H, 4)                      # the sample only touches a few heads
+    sub = W.scaled(cfg, H=heads)
+    Qb, Kb, Vb = W.qkv_bits(sub)
+    bm = W.layer_mask(sub)
+    cores = oracle.num_threads()
+    # size one step at ~2.5 s of CPU work
+    dt, fl, _ = oracle_sample_time(sub, Qb, Kb, Vb, bm, cores)
+    n = int(max(1, min(16 * cores, round(cores * 2.5 / max(dt, 1e-3)))))
+    for _ in range(args.warmup):
+        oracle_sample_time(sub, Qb, Kb, Vb, bm, max(1, n // 4))
+    tot_t = tot_f = 0.0
+    for s in range(args.steps):
+        dt, fl, _ = oracle_sample_time(sub, Qb, Kb, Vb, bm, n, seed=s)
+        tot_t += dt
+        tot_f += fl
+    val = tot_f / tot_t / 1e12
+    sample = f"{n} random (head, query-block) items of {cfg.name} per step, fp64 oracle"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": cfg.name, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------------------------
+# the CUDA path
+# --------------------------------------------------------------------------------------------------
+def run_chorus(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_25040_b200 import binding as B
+    from paper_2606_25040_b200 import workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    B.lib()  # fail loudly if the extension is missing
+
+    cfg = get_cfg(args.workload)
+    peaks = load_peaks()
+    Qb, Kb, Vb = W.qkv_bits(cfg)
+    bm = W.layer_mask(cfg)
+    density = W.mask_density(bm, cfg.nk)
+    flops_attn = attn_flops(cfg, density)
+
+    to_bf16 = lambda x: torch.from_numpy(x.view(np.int16)).view(torch.bfloat16)
+    hQ, hK, hV = (to_bf16(x).pin_memory() for x in (Qb, Kb, Vb))
+    hM = torch.from_numpy(bm[None].view(np.int32)).pin_memory()
+    hO = torch.empty((cfg.B, cfg.N, cfg.H, cfg.d), dtype=torch.bfloat16).pin_memory()
+    dQ, dK, dV, dM = (x.to(dev) for x in (hQ, hK, hV, hM))
+    dO = torch.empty_like(dQ)
+    rows = cfg.H * cfg.nq
+    row_ptr = torch.empty(rows + 1, dtype=torch.int32, device=dev)
+    col_idx = torch.empty(rows * cfg.nk, dtype=torch.int32, device=dev)  # upper bound: no D2H read of nnz
+    ws = torch.empty(max(4, B.mask_to_index_workspace_bytes(1, cfg.H, cfg.nq, cfg.nk)), dtype=torch.uint8, device=dev)
+    has_fp8 = args.fp8
+    if has_fp8:
+        q8 = B.chorus_quantize_fp8(dQ, dK, dV)
+        dO8 = torch.empty_like(dQ)
+    stream = torch.cuda.current_stream()
+
+    def step(ev=None):
+        B.chorus_mask_to_index(dM, cfg.nk, row_ptr=row_ptr, col_idx=col_idx, workspace=ws)
+        if ev: ev[0].record(stream)
+        B.chorus_block_sparse_attn_fwd(dQ, dK, dV, row_ptr, col_idx, cfg.scale, O=dO)
+        if ev: ev[1].record(stream)
+        if has_fp8:
+            B.chorus_quantize_fp8(dQ, dK, dV, out=q8)
+            if ev: ev[2].record(stream)
+            B.chorus_block_sparse_attn_fwd(q8[0], q8[1], q8[2], row_ptr, col_idx, cfg.scale,
+                                           dtype=B.CHORUS_FP8_E4M3, O=dO8, fp8_scales=q8[3:])
+            if ev: ev[3].record(stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    K = args.steps
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
+    e_start = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    e_end = torch.cuda.Event(enable_timing=True)
+    B.chorus_reset_launch_count()
+    for k in range(K):
+        e_start[k].record(stream)
+        step(evs[k])
+    e_end.record(stream)
+    barrier()
+    launches = B.chorus_launch_count()
+    total_ms = e_start[0].elapsed_time(e_end)
+    dec_ms = statistics.mean(e_start[k].elapsed_time(evs[k][0]) for k in range(K))
+    attn_ms = statistics.mean(evs[k][0].elapsed_time(evs[k][1]) for k in range(K))
+    attn_ms_min = min(evs[k][0].elapsed_time(evs[k][1]) for k in range(K))
+    if has_fp8:
+        quant_ms = statistics.mean(evs[k][1].elapsed_time(evs[k][2]) for k in range(K))
+        attn8_ms = statistics.mean(evs[k][2].elapsed_time(evs[k][3]) for k in range(K))
+
+    # end-to-end through the ABI with HOST buffers: H2D of Q, K, V and the mask, D2H of O, per step
+    def e2e_step():
+        dQ.copy_(hQ, non_blocking=True); dK.copy_(hK, non_blocking=True); dV.copy_(hV, non_blocking=True)
+        dM.copy_(hM, non_blocking=True)
+        step()
+        hO.copy_(dO, non_blocking=True)
+    e2e_steps = max(2, min(K, 5))
+    e2e_step()
+    barrier()
+    a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(e2e_steps):
+        e2e_step()
+    b_.record(stream)
+    barrier()
+    e2e_ms = a.elapsed_time(b_) / e2e_steps
+    clocks = sampler.stop() if rank == 0 else None
+
+    t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = t.tolist()
+    ms_per_step = total_ms / K
+    step_flops = flops_attn * (2 if has_fp8 else 1)
+    value = world * step_flops / (ms_per_step * 1e-3) / 1e12
+    e2e_val = world * step_flops / (e2e_ms * 1e-3) / 1e12
+
+    if rank == 0:
+        achieved = flops_attn / (attn_ms * 1e-3) / 1e12
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+        if os.path.exists(tp):
+            traffic = json.load(open(tp)).get(f"{cfg.name}_bf16_attn_dram_bytes_per_launch")
+        nnz = int(round(density * rows * cfg.nk))
+        dec_bytes = 4 * (rows * cfg.words) + 4 * (rows + 1) + 4 * nnz
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "bf16" + ("+fp8_e4m3" if has_fp8 else ""),
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "B": cfg.B, "H": cfg.H, "N": cfg.N, "d": cfg.d,
+                       "block": "128q x 64k", "density": density, "multi_gpu": "replicas only",
+                       "l2": "inputs larger than L2 (Q+K+V+O = %.2f GB per step)" % (4 * Qb.nbytes / 1e9),
+                       "step": "mask_to_index -> attn_fwd(bf16)" + (" -> quantize_fp8 -> attn_fwd(fp8)" if has_fp8 else "")},
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms,
+                    "h2d_bytes_per_step": int(3 * Qb.nbytes + bm.nbytes), "d2h_bytes_per_step": int(Qb.nbytes)},
+            "gpu_launches": int(launches),
+            "roofline": {"kernel": "attn_fwd bf16", "bound": "tensor", "achieved": achieved,
+                         "peak": peaks["bf16"], "unit": "TFLOP/s", "frac": achieved / peaks["bf16"],
+                         "traffic": traffic, "peak_source": peaks["source"] + " (burst cuBLAS bf16)",
+                         "frac_of_sustained": achieved / peaks["bf16_sustained"] if peaks["bf16_sustained"] else None,
+                         "frac_of_datasheet_2250": achieved / 2250.0,
+                         "ms": attn_ms, "ms_min": attn_ms_min, "flops_per_launch": flops_attn},
+            "breakdown": {"decode_ms": dec_ms, "decode_GBps": dec_bytes / (dec_ms * 1e-3) / 1e9,
+                          "decode_frac_of_hbm": dec_bytes / (dec_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                          "attn_bf16_ms": attn_ms, "attn_bf16_TFLOPs": achieved,
+                          "routing_overhead_ratio": dec_ms / (dec_ms + attn_ms)},
+        }
+        if has_fp8:
+            a8 = flops_attn / (attn8_ms * 1e-3) / 1e12
+            line["breakdown"].update({"quantize_ms": quant_ms, "attn_fp8_ms": attn8_ms, "attn_fp8_TFLOPs": a8,
+                                      "attn_fp8_frac_of_2x_bf16_peak": a8 / (2 * peaks["bf16"]),
+                                      "attn_fp8_frac_of_datasheet_4500": a8 / 4500.0})
+        if world == 1 and not args.no_cpu_baseline:
+            heads = min(cfg.H, 4)
+            line["cpu_baseline"] = cpu_baseline(W.scaled(cfg, H=heads), Qb[:, :, :heads].copy(),
+                                                Kb[:, :, :heads].copy(), Vb[:, :, :heads].copy(), bm[:heads])
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="chorus", choices=["chorus", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg4"])
+    ap.add_argument("--fp8", action="store_true", default=False)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "chorus" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_chorus(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -13,13 +13,20 @@ from paper_2606_25040_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 
-def compare(cfg, Q, K, V, bm, items, scale=None, tight=True):
+def compare(cfg, Q, K, V, bm, items, scale=None, tight=True, stress=False):
     scale = cfg.scale if scale is None else scale
     O = gpu_attention(Q, K, V, bm, cfg.nk, scale)
     assert not np.isnan(O).any()
     ref = oracle_items(Q, K, V, bm, scale, items)
     got = gather_items(O, items, cfg.N)
     mx, mean, relfro, cos = err_stats(got, ref)
+    if stress:
+        # x8 rows give outputs of magnitude ~25, where the bf16 OUTPUT format alone rounds by
+        # 2^-9 |O| ~ 0.05: the absolute 2e-2 bound is stated for N(0,1) inputs (north_star), so it
+        # is applied to the error in excess of two bf16 roundings
+        assert np.all(np.abs(got - ref) <= BF16_MAX + 2.0 ** -8 * np.abs(ref)), mx
+        assert mean <= BF16_MEAN and relfro <= BF16_RELFRO, (mean, relfro)
+        return O
     assert mx <= BF16_MAX and mean <= BF16_MEAN, (mx, mean)
     if tight:
         assert mx <= BF16_MAX_TIGHT and relfro <= BF16_RELFRO, (mx, relfro)
@@ -119,14 +126,14 @@ def test_spike_and_pruned_block_probe():
     K2 = K.copy()
     rows = [5, 1000, cfg.N - 1]
     targets = []
-    for i in rows:
+    for n_spike, i in enumerate(rows):
         qb = i // 128
         kept = np.nonzero(keep[qb])[0]
         kb = kept[-1] if i == cfg.N - 1 else kept[len(kept) // 2]
         if i == cfg.N - 1:
             keep[qb, cfg.nk - 1] = True
             kb = cfg.nk - 1                      # spike inside the ragged last key block
-        j = min(64 * kb + 3, cfg.N - 1)
+        j = min(64 * kb + 3 + 7 * n_spike, cfg.N - 1)   # distinct keys even if rows share kb
         q = qf[0, i, 0]
         K2[0, j, 0] = W.bf16_bits_from_f32((60.0 / cfg.scale * q / (q @ q)).astype(np.float32))
         targets.append((i, j))
@@ -160,7 +167,7 @@ def test_cfg4_720p_stress_rows_sampled_blocks():
     Q, K, V = W.qkv_bits(cfg)
     bm = W.layer_mask(cfg)
     items = sample_items(cfg.H, cfg.nq, 5, seed=1, always=[(0, 3, cfg.nq - 1)])
-    compare(cfg, Q, K, V, bm, items, tight=False)
+    compare(cfg, Q, K, V, bm, items, stress=True)
 
 
 def test_density_sweep_one_head():
