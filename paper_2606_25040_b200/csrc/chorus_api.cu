@@ -195,7 +195,7 @@ chorus_status chorus_block_sparse_attn_fwd(const void* Q, const void* K, const v
     if ((st = make_tmap(&tmV, V, eb, s.B, s.H, s.N, s.d, s.v_stride_b, s.v_stride_n, s.v_stride_h,
                         cols, CHORUS_BLOCK_K, "V")) != CHORUS_OK) return st;
     if ((st = make_tmap(&tmO, O, 2, s.B, s.H, s.N, s.d, s.o_stride_b, s.o_stride_n, s.o_stride_h,
-                        64, 32, "O")) != CHORUS_OK) return st;
+                        64, CHORUS_BLOCK_Q, "O")) != CHORUS_OK) return st;
 
     AttnParams p;
     p.row_ptr = row_ptr;
