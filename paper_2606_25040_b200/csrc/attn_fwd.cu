@@ -4,19 +4,19 @@
 // Persistent, warp-specialised kernel, one CTA (384 threads) per SM:
 //   warp 8        TMA producer: Q tile once per work item, then the kept K / V tiles of the CSR row,
 //                 two 64-key tiles ("a pair") per pipeline stage, 128-byte swizzle
-//   warp 9        MMA issuer (one thread): S = Q K^T (M=128, N=128, K=128) into tensor memory,
-//                 O += P V (M=128, N=128, K=128) with P as the TMEM A operand and V as an MN-major
+//   warp 9        MMA issuer (one thread): S = Q K^T (M=128, N=128, K=128) into one of THREE S
+//                 buffers in tensor memory, up to two pairs ahead of the softmax; O += P V
+//                 (M=128, N=128, K=128) with P as the TMEM A operand and V as an MN-major
 //                 shared-memory B operand
-//   warps 0-3     softmax warpgroup of stream 0 (pairs 0, 2, 4, ...)
-//   warps 4-7     softmax warpgroup of stream 1 (pairs 1, 3, 5, ...)
+//   warps 0-7     softmax.  Warp w owns TMEM lanes 32*(w%4).. (one query row per thread) and the
+//                 64 score columns of tile (w/4) of the pair: warps w and w+4 share their rows'
+//                 running max through shared memory and a 64-thread named barrier per pair.
 // A work item is one (batch, head, 128-row query block).  Its kept tiles are paired (any two kept
-// tiles, not necessarily adjacent keys) so that QK^T runs at N=128; even and odd pairs form two
-// independent online-softmax streams with their own S and O accumulators in tensor memory
-// (S0 S1 O0 O1 = 4 x 128 columns), so the tensor pipe works on one stream while the other stream's
-// warpgroup does its exponentials.  Each thread owns one query row (TMEM lane): row max and row sum
-// need no shuffles.  O is rescaled lazily (only when the row max grows by more than 2^8).  The two
-// streams are merged in the epilogue, normalised, converted to bf16, staged in shared memory and
-// written with TMA stores (coalesced 128-byte rows; rows beyond N are clipped by the tensor map).
+// tiles, not necessarily adjacent keys) so that QK^T runs at N=128.  P (bf16) overwrites the first
+// half of each warp's own S columns.  O (fp32, 128 columns of TMEM) is rescaled lazily: only when
+// a row max grows by more than 2^8 over the reference that the accumulators currently use.  The
+// epilogue normalises, converts to bf16, stages in shared memory and writes with TMA stores
+// (coalesced 128-byte rows; rows beyond N are clipped by the tensor map).
 #include <cuda_bf16.h>
 
 #include "chorus_internal.h"
@@ -28,7 +28,7 @@ namespace {
 using namespace ptx;
 
 constexpr int BQ = 128, BK = 64;
-constexpr int KSTAGES = 2, VSTAGES = 3;
+constexpr int KSTAGES = 2, VSTAGES = 3, SBUFS = 3;
 constexpr int NUM_THREADS = 384;
 constexpr int PRODUCER_WARP = 8, MMA_WARP = 9;
 
@@ -37,8 +37,8 @@ constexpr uint32_t SQ_OFF = 0;                         // Q : 2 slabs [128 rows]
 constexpr uint32_t SK_OFF = 32768;                     // K : KSTAGES x 2 slabs [128 keys][128 B]
 constexpr uint32_t SV_OFF = SK_OFF + KSTAGES * 32768;  // V : VSTAGES x 2 slabs [128 keys][128 B]
 constexpr uint32_t SO_OFF = SV_OFF + VSTAGES * 32768;  // O staging: 2 slabs [128 rows][128 B]
-constexpr uint32_t SML_OFF = SO_OFF + 32768;           // (m, l) exchange: 2 x 128 x float2  2 KB
-constexpr uint32_t BAR_OFF = SML_OFF + 2048;
+constexpr uint32_t XCH_OFF = SO_OFF + 32768;           // row max / row sum exchange [2 parity][2 half][128] f32
+constexpr uint32_t BAR_OFF = XCH_OFF + 2048;
 constexpr uint32_t SMEM_BYTES = BAR_OFF + 256;
 static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
 
@@ -46,17 +46,20 @@ static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of
 enum : uint32_t {
     B_Q_FULL = 0, B_Q_EMPTY = 1, B_K_FULL = 2, B_K_EMPTY = B_K_FULL + KSTAGES,
     B_V_FULL = B_K_EMPTY + KSTAGES, B_V_EMPTY = B_V_FULL + VSTAGES, B_S_FULL = B_V_EMPTY + VSTAGES,
-    B_P_READY = B_S_FULL + 2, B_O_FULL = B_P_READY + 2, B_O_FREE = B_O_FULL + 1,
+    B_P_READY = B_S_FULL + SBUFS, B_PV_DONE = B_P_READY + SBUFS, B_O_FREE = B_PV_DONE + SBUFS,
     B_COUNT = B_O_FREE + 1
 };
 static_assert(B_COUNT * 8 + 8 <= 256, "barrier area too small");
 
-// tensor-memory map (columns)
-constexpr uint32_t TM_S0 = 0, TM_S1 = 128, TM_O0 = 256, TM_O1 = 384, TM_COLS = 512;
+// tensor-memory map (columns): three S buffers and the O accumulator
+constexpr uint32_t TM_S = 0, TM_O = 384, TM_COLS = 512;
+
+// named barriers: 0 = __syncthreads, 1..4 = warp pair (w, w+4), 5..6 = column-half warpgroup
+constexpr uint32_t NB_PAIR = 1, NB_HALF = 5;
 
 constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units: p stays below 2^8
 
-__device__ __forceinline__ void setmaxnreg_inc_224() { asm volatile("setmaxnreg.inc.sync.aligned.u32 224;"); }
+__device__ __forceinline__ void setmaxnreg_inc_216() { asm volatile("setmaxnreg.inc.sync.aligned.u32 216;"); }
 __device__ __forceinline__ void setmaxnreg_dec_56() { asm volatile("setmaxnreg.dec.sync.aligned.u32 56;"); }
 
 struct Item {
@@ -75,6 +78,8 @@ __device__ __forceinline__ Item get_item(const AttnParams& p, int idx) {
     return it;
 }
 
+__device__ __forceinline__ float max3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
+
 template <bool kFp8>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
@@ -90,7 +95,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const uint32_t bars = base + BAR_OFF;
     auto bar = [&](uint32_t i) { return bars + 8u * i; };
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gbase + BAR_OFF + 8 * B_COUNT);
-    float2* sml = reinterpret_cast<float2*>(gbase + SML_OFF);
+    volatile float* xch = reinterpret_cast<volatile float*>(gbase + XCH_OFF);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_items = p.B * p.H * p.nq;
@@ -100,8 +105,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(bar(B_Q_EMPTY), 1);
         for (int i = 0; i < KSTAGES; ++i) { mbar_init(bar(B_K_FULL + i), 1); mbar_init(bar(B_K_EMPTY + i), 1); }
         for (int i = 0; i < VSTAGES; ++i) { mbar_init(bar(B_V_FULL + i), 1); mbar_init(bar(B_V_EMPTY + i), 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(bar(B_S_FULL + i), 1); mbar_init(bar(B_P_READY + i), 4); }
-        mbar_init(bar(B_O_FULL), 1);
+        for (int i = 0; i < SBUFS; ++i) {
+            mbar_init(bar(B_S_FULL + i), 1);
+            mbar_init(bar(B_P_READY + i), 8);
+            mbar_init(bar(B_PV_DONE + i), 1);
+        }
         mbar_init(bar(B_O_FREE), 8);
         fence_mbar_init();
     }
@@ -118,20 +126,20 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // ======================= producer / MMA warpgroup ==========================================
         setmaxnreg_dec_56();
         if (warp == PRODUCER_WARP && lane == 0) {
-            uint32_t kcnt = 0, vcnt = 0, icnt = 0;
+            uint32_t g = 0, icnt = 0;   // pairs and non-empty items issued so far
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
                 const Item it = get_item(p, idx);
-                if (it.nt == 0) continue;   // empty rows touch no barrier: icnt counts non-empty items
+                if (it.nt == 0) continue;   // empty rows touch no barrier
                 mbar_wait(bar(B_Q_EMPTY), (icnt & 1) ^ 1);
                 mbar_arrive_expect_tx(bar(B_Q_FULL), 32768);
                 tma_load_4d(sQ, &tmQ, bar(B_Q_FULL), 0, it.qb * BQ, it.h, it.b);
                 tma_load_4d(sQ + 16384, &tmQ, bar(B_Q_FULL), 64, it.qb * BQ, it.h, it.b);
-                for (int j = 0; j < it.np; ++j) {
+                for (int j = 0; j < it.np; ++j, ++g) {
                     const int ntile = (2 * j + 1 < it.nt) ? 2 : 1;
                     const int kb0 = __ldg(p.col_idx + it.r0 + 2 * j);
                     const int kb1 = (ntile == 2) ? __ldg(p.col_idx + it.r0 + 2 * j + 1) : 0;
                     {
-                        const uint32_t st = kcnt % KSTAGES, ph = (kcnt / KSTAGES) & 1;
+                        const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1;
                         mbar_wait(bar(B_K_EMPTY + st), ph ^ 1);
                         mbar_arrive_expect_tx(bar(B_K_FULL + st), ntile * 16384);
                         const uint32_t dst = sK + st * 32768;
@@ -141,10 +149,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             tma_load_4d(dst + 8192, &tmK, bar(B_K_FULL + st), 0, kb1 * BK, it.h, it.b);
                             tma_load_4d(dst + 16384 + 8192, &tmK, bar(B_K_FULL + st), 64, kb1 * BK, it.h, it.b);
                         }
-                        ++kcnt;
                     }
                     {
-                        const uint32_t st = vcnt % VSTAGES, ph = (vcnt / VSTAGES) & 1;
+                        const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1;
                         mbar_wait(bar(B_V_EMPTY + st), ph ^ 1);
                         mbar_arrive_expect_tx(bar(B_V_FULL + st), ntile * 16384);
                         const uint32_t dst = sV + st * 32768;
@@ -154,7 +161,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             tma_load_4d(dst + 8192, &tmV, bar(B_V_FULL + st), 0, kb1 * BK, it.h, it.b);
                             tma_load_4d(dst + 16384 + 8192, &tmV, bar(B_V_FULL + st), 64, kb1 * BK, it.h, it.b);
                         }
-                        ++vcnt;
                     }
                 }
                 ++icnt;
@@ -163,171 +169,181 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             constexpr uint32_t IDESC_S128 = make_idesc(1, 1, 128, 128, 0, 0);
             constexpr uint32_t IDESC_S64 = make_idesc(1, 1, 128, 64, 0, 0);
             constexpr uint32_t IDESC_PV = make_idesc(1, 1, 128, 128, 0, 1);
-            uint32_t kcnt = 0, vcnt = 0, icnt = 0, pcnt[2] = {0, 0};
+            const uint64_t dQ = smem_desc_sw128(sQ, 16, 1024);
+            const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
+            const uint64_t dV = smem_desc_sw128(sV, 16384, 1024);
+            uint32_t g0 = 0, icnt = 0;   // pairs before this item, non-empty items so far
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
                 const Item it = get_item(p, idx);
                 if (it.nt == 0) continue;
-                auto issue_pv = [&](int jj) {
-                    const int s = jj & 1;
-                    const int ntile = (2 * jj + 1 < it.nt) ? 2 : 1;
-                    mbar_wait(bar(B_P_READY + s), pcnt[s] & 1);
-                    ++pcnt[s];
-                    const uint32_t st = vcnt % VSTAGES, ph = (vcnt / VSTAGES) & 1;
-                    mbar_wait(bar(B_V_FULL + st), ph);
-                    tc_fence_after();
-                    const uint32_t tP = tmem + (s ? TM_S1 : TM_S0), tO = tmem + (s ? TM_O1 : TM_O0);
-                    const int nks = 4 * ntile;
-                    for (int ks = 0; ks < nks; ++ks) {
-                        const uint64_t db = smem_desc_sw128(sV + st * 32768 + ks * 2048, 16384, 1024);
-                        mma_f16_ts(tO, tP + ks * 8, db, IDESC_PV, (jj >= 2) || (ks > 0));
-                    }
-                    tc_commit(bar(B_V_EMPTY + st));
-                    ++vcnt;
-                };
                 mbar_wait(bar(B_Q_FULL), icnt & 1);
-                mbar_wait(bar(B_O_FREE), (icnt & 1) ^ 1);
-                for (int j = 0; j < it.np; ++j) {
-                    const int s = j & 1;
-                    const int ntile = (2 * j + 1 < it.nt) ? 2 : 1;
-                    const uint32_t st = kcnt % KSTAGES, ph = (kcnt / KSTAGES) & 1;
-                    mbar_wait(bar(B_K_FULL + st), ph);
-                    tc_fence_after();
-                    const uint32_t tS = tmem + (s ? TM_S1 : TM_S0);
-                    const uint32_t idesc = (ntile == 2) ? IDESC_S128 : IDESC_S64;
+                for (int jj = 0; jj < it.np + 2; ++jj) {
+                    if (jj < it.np) {   // S[g % 3] = Q K^T of pair jj (runs up to two pairs ahead)
+                        const uint32_t g = g0 + jj;
+                        const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1, sb = g % SBUFS;
+                        const int ntile = (2 * jj + 1 < it.nt) ? 2 : 1;
+                        mbar_wait(bar(B_K_FULL + st), ph);
+                        tc_fence_after();
+                        const uint32_t tS = tmem + TM_S + sb * 128;
+                        const uint32_t idesc = (ntile == 2) ? IDESC_S128 : IDESC_S64;
+                        const uint64_t dKs = dK + ((st * 32768u) >> 4);
 #pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) {
-                        const uint32_t off = (ks >> 2) * 16384 + (ks & 3) * 32;
-                        const uint64_t da = smem_desc_sw128(sQ + off, 16, 1024);
-                        const uint64_t db = smem_desc_sw128(sK + st * 32768 + off, 16, 1024);
-                        mma_f16_ss(tS, da, db, idesc, ks > 0);
+                        for (int ks = 0; ks < 8; ++ks) {
+                            const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
+                            mma_f16_ss(tS, dQ + off, dKs + off, idesc, ks > 0);
+                        }
+                        tc_commit(bar(B_K_EMPTY + st));
+                        tc_commit(bar(B_S_FULL + sb));
+                        if (jj == it.np - 1) tc_commit(bar(B_Q_EMPTY));
                     }
-                    tc_commit(bar(B_K_EMPTY + st));
-                    tc_commit(bar(B_S_FULL + s));
-                    ++kcnt;
-                    if (j == it.np - 1) tc_commit(bar(B_Q_EMPTY));
-                    if (j >= 1) issue_pv(j - 1);
+                    if (jj >= 2) {      // O += P V of pair jj - 2
+                        const int jp = jj - 2;
+                        const uint32_t g = g0 + jp;
+                        const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1, sb = g % SBUFS;
+                        const int ntile = (2 * jp + 1 < it.nt) ? 2 : 1;
+                        mbar_wait(bar(B_P_READY + sb), (g / SBUFS) & 1);
+                        mbar_wait(bar(B_V_FULL + st), ph);
+                        if (jp == 0) mbar_wait(bar(B_O_FREE), (icnt & 1) ^ 1);
+                        tc_fence_after();
+                        const uint32_t tP = tmem + TM_S + sb * 128, tO = tmem + TM_O;
+                        const uint64_t dVs = dV + ((st * 32768u) >> 4);
+#pragma unroll
+                        for (int ks = 0; ks < 8; ++ks) {
+                            if (ks < 4 * ntile) {
+                                // P of tile 0 lives in S columns [0, 32), P of tile 1 in [64, 96)
+                                const uint32_t ta = tP + (ks >> 2) * 64 + (ks & 3) * 8;
+                                mma_f16_ts(tO, ta, dVs + ((ks * 2048u) >> 4), IDESC_PV, (jp > 0) || (ks > 0));
+                            }
+                        }
+                        tc_commit(bar(B_V_EMPTY + st));
+                        tc_commit(bar(B_PV_DONE + sb));
+                    }
                 }
-                issue_pv(it.np - 1);
-                tc_commit(bar(B_O_FULL));
+                g0 += it.np;
                 ++icnt;
             }
         }
     } else {
-        // ======================= softmax warpgroups =================================================
-        setmaxnreg_inc_224();
-        const int s = warp >> 2;                 // stream
+        // ======================= softmax warps ======================================================
+        setmaxnreg_inc_216();
+        const int s = warp >> 2;                 // which tile of the pair: score columns [64 s, 64 s + 64)
         const int wq = warp & 3;                 // TMEM lane quarter
         const int row = wq * 32 + lane;          // query row inside the block == TMEM lane
         const uint32_t tlane = tmem + (static_cast<uint32_t>(wq * 32) << 16);
-        const uint32_t tS = tlane + (s ? TM_S1 : TM_S0);
-        const uint32_t tO = tlane + (s ? TM_O1 : TM_O0);
+        const uint32_t tO = tlane + TM_O + s * 64;   // this warp rescales / finalises O columns [64 s, 64 s + 64)
         const float sl2 = p.scale_log2;
-        uint32_t scnt = 0, icnt = 0;
+        uint32_t g = 0;                          // pairs processed so far (all items)
+        uint32_t xc = 0;                         // exchanges so far: slot parity (two slots, one barrier each)
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
             const Item it = get_item(p, idx);
-            float m = -INFINITY, l = 0.f;
-            if (it.nt > 0) {
-                for (int j = s; j < it.np; j += 2) {
-                    mbar_wait(bar(B_S_FULL + s), scnt & 1);
-                    ++scnt;
-                    tc_fence_after();
-                    uint32_t sv[128];
+            float m_ref = -INFINITY, l0 = 0.f, l1 = 0.f;
+            for (int j = 0; j < it.np; ++j, ++g) {
+                const uint32_t sb = g % SBUFS;
+                const uint32_t tS = tlane + TM_S + sb * 128 + s * 64;
+                int valid = BK;                  // valid keys in this warp's tile of the pair
+                if (j == it.np - 1) {            // only the last pair can be odd or hold the ragged key block
+                    if (2 * j + s < it.nt) valid = min(BK, p.N - __ldg(p.col_idx + it.r0 + 2 * j + s) * BK);
+                    else valid = 0;
+                }
+                mbar_wait(bar(B_S_FULL + sb), (g / SBUFS) & 1);
+                tc_fence_after();
+                uint32_t sv[64];
+                float mx = -INFINITY;
+                if (valid > 0) {
                     tmem_ld32(tS, *reinterpret_cast<uint32_t(*)[32]>(sv));
                     tmem_ld32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(sv + 32));
-                    tmem_ld32(tS + 64, *reinterpret_cast<uint32_t(*)[32]>(sv + 64));
-                    tmem_ld32(tS + 96, *reinterpret_cast<uint32_t(*)[32]>(sv + 96));
                     tc_wait_ld();
-                    if (j == it.np - 1) {  // only the last pair can be odd or hold the ragged key block
-                        const int kb0 = __ldg(p.col_idx + it.r0 + 2 * j);
-                        const int v0 = min(BK, p.N - kb0 * BK);
-                        int v1 = 0;
-                        if (2 * j + 1 < it.nt) {
-                            const int kb1 = __ldg(p.col_idx + it.r0 + 2 * j + 1);
-                            v1 = min(BK, p.N - kb1 * BK);
-                        }
-                        if (v0 < BK || v1 < BK) {
+                    if (valid < BK) {
 #pragma unroll
-                            for (int k = 0; k < 64; ++k) {
-                                if (k >= v0) sv[k] = 0xff800000u;       // -inf
-                                if (k >= v1) sv[64 + k] = 0xff800000u;
-                            }
+                        for (int k = 0; k < 64; ++k)
+                            if (k >= valid) sv[k] = 0xff800000u;   // -inf
+                    }
+                    float a0 = -INFINITY, a1 = -INFINITY, a2 = -INFINITY, a3 = -INFINITY;
+#pragma unroll
+                    for (int k = 0; k < 64; k += 8) {
+                        a0 = max3(a0, __uint_as_float(sv[k]), __uint_as_float(sv[k + 1]));
+                        a1 = max3(a1, __uint_as_float(sv[k + 2]), __uint_as_float(sv[k + 3]));
+                        a2 = max3(a2, __uint_as_float(sv[k + 4]), __uint_as_float(sv[k + 5]));
+                        a3 = max3(a3, __uint_as_float(sv[k + 6]), __uint_as_float(sv[k + 7]));
+                    }
+                    mx = fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)) * sl2;
+                }
+                // the row max of the pair: exchange with the warp that holds the other 64 columns
+                const uint32_t par = (xc++) & 1;
+                xch[(par * 2 + s) * 128 + row] = mx;
+                named_bar_sync(NB_PAIR + wq, 64);
+                const float mt = fmaxf(mx, xch[(par * 2 + (s ^ 1)) * 128 + row]);
+                if (__any_sync(0xffffffffu, mt > m_ref + RESCALE_THRESHOLD)) {
+                    // identical decision in both warps of the pair (same mt, same m_ref per row)
+                    const float m_new = fmaxf(m_ref, mt);
+                    const float alpha = ex2(m_ref - m_new);   // m_ref = -inf (first pair) -> 0
+                    l0 *= alpha;
+                    l1 *= alpha;
+                    m_ref = m_new;
+                    if (j > 0) {
+                        // O holds pairs 0..j-1 under the old reference; wait for P V of pair j-1.
+                        // (S_FULL of pair g implies P V of pair g-3 is complete, so the barrier of
+                        // buffer (g-1) % 3 is at most one phase behind: the parity wait is exact.)
+                        mbar_wait(bar(B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
+                        tc_fence_after();
+#pragma unroll 1
+                        for (int c = 0; c < 2; ++c) {
+                            uint32_t o[32];
+                            tmem_ld32(tO + c * 32, o);
+                            tc_wait_ld();
+#pragma unroll
+                            for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * alpha);
+                            tmem_st32(tO + c * 32, o);
                         }
                     }
-                    float mx = -INFINITY;
-#pragma unroll
-                    for (int k = 0; k < 128; ++k) mx = fmaxf(mx, __uint_as_float(sv[k]));
-                    const float m_new = fmaxf(m, mx * sl2);
-                    if (__any_sync(0xffffffffu, m_new > m + RESCALE_THRESHOLD)) {
-                        const float alpha = ex2(m - m_new);   // m = -inf (first pair) -> 0
-                        l *= alpha;
-                        m = m_new;
-                        if (j >= 2) {
-                            // previous P V of this stream has completed (S_FULL tracks all earlier MMAs)
-#pragma unroll
-                            for (int c = 0; c < 4; ++c) {
-                                uint32_t o[32];
-                                tmem_ld32(tO + c * 32, o);
-                                tc_wait_ld();
-#pragma unroll
-                                for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * alpha);
-                                tmem_st32(tO + c * 32, o);
-                            }
-                        }
-                    }
-                    const float neg_m = -m;
-                    float sum0 = 0.f, sum1 = 0.f;
+                }
+                if (valid > 0) {
+                    const float neg_m = -m_ref;
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
-                        uint32_t pk[16];
+                        uint32_t pk[8];
 #pragma unroll
-                        for (int k = 0; k < 16; ++k) {
-                            const float p0 = ex2(fmaf(__uint_as_float(sv[c * 32 + 2 * k]), sl2, neg_m));
-                            const float p1 = ex2(fmaf(__uint_as_float(sv[c * 32 + 2 * k + 1]), sl2, neg_m));
-                            sum0 += p0;
-                            sum1 += p1;
+                        for (int k = 0; k < 8; ++k) {
+                            const float p0 = ex2(fmaf(__uint_as_float(sv[c * 16 + 2 * k]), sl2, neg_m));
+                            const float p1 = ex2(fmaf(__uint_as_float(sv[c * 16 + 2 * k + 1]), sl2, neg_m));
+                            l0 += p0;
+                            l1 += p1;
                             pk[k] = pack_bf16x2(p0, p1);
                         }
-                        tmem_st16(tS + c * 16, pk);
+                        tmem_st8(tS + c * 8, pk);   // P: bf16 pairs over this warp's first 32 S columns
                     }
-                    l += sum0 + sum1;
-                    tc_wait_st();
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar(B_P_READY + s));
                 }
+                tc_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_P_READY + sb));
             }
-            // ---------------- epilogue: merge the two streams, normalise, store ------------------
-            sml[s * 128 + row] = make_float2(m, l);
-            if (lane == 0 && wq == 0) tma_store_wait_read();   // staging slab s free again
-            named_bar_sync(1, 256);
-            const float2 other = sml[(s ^ 1) * 128 + row];
-            named_bar_sync(4, 256);   // both reads done before either warpgroup rewrites its slot
-            const float m_all = fmaxf(m, other.x);
-            const float a_self = (m == -INFINITY) ? 0.f : ex2(m - m_all);
-            const float a_oth = (other.x == -INFINITY) ? 0.f : ex2(other.x - m_all);
-            const float L = l * a_self + other.y * a_oth;
+            // ---------------- epilogue: normalise, convert, store --------------------------------
+            const float l = l0 + l1;
+            const uint32_t par = (xc++) & 1;
+            xch[(par * 2 + s) * 128 + row] = l;
+            if (lane == 0 && wq == 0) tma_store_wait_read();   // staging slab s is free again
+            named_bar_sync(NB_PAIR + wq, 64);
+            const float L = l + xch[(par * 2 + (s ^ 1)) * 128 + row];
             const float inv = (L > 0.f) ? 1.f / L : 0.f;
-            const float w_s0 = (s == 0 ? a_self : a_oth) * inv, w_s1 = (s == 0 ? a_oth : a_self) * inv;
-            const bool has0 = it.np > 0, has1 = it.np > 1;
+            named_bar_sync(NB_HALF + s, 128);                  // staging free for the whole warpgroup
             if (it.nt > 0) {
-                mbar_wait(bar(B_O_FULL), icnt & 1);
-                ++icnt;
+                mbar_wait(bar(B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
                 tc_fence_after();
             }
-            // this warpgroup finalises output columns [64 s, 64 s + 64)
             const uint32_t srow = sO + s * 16384 + row * 128;
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
-                uint32_t o0[32], o1[32];
-                if (has0) tmem_ld32(tlane + TM_O0 + s * 64 + c * 32, o0);
-                if (has1) tmem_ld32(tlane + TM_O1 + s * 64 + c * 32, o1);
-                if (has0) tc_wait_ld();
+                uint32_t o[32];
+                if (it.nt > 0) {
+                    tmem_ld32(tO + c * 32, o);
+                    tc_wait_ld();
+                }
                 uint32_t pk[16];
 #pragma unroll
                 for (int k = 0; k < 16; ++k) {
                     float x0 = 0.f, x1 = 0.f;
-                    if (has0) { x0 = __uint_as_float(o0[2 * k]) * w_s0; x1 = __uint_as_float(o0[2 * k + 1]) * w_s0; }
-                    if (has1) { x0 = fmaf(__uint_as_float(o1[2 * k]), w_s1, x0); x1 = fmaf(__uint_as_float(o1[2 * k + 1]), w_s1, x1); }
+                    if (it.nt > 0) { x0 = __uint_as_float(o[2 * k]) * inv; x1 = __uint_as_float(o[2 * k + 1]) * inv; }
                     pk[k] = pack_bf16x2(x0, x1);
                 }
 #pragma unroll
@@ -344,7 +360,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 if (lane == 0) mbar_arrive(bar(B_O_FREE));
             }
             fence_proxy_async_smem();
-            named_bar_sync(2 + s, 128);
+            named_bar_sync(NB_HALF + s, 128);
             if (lane == 0 && wq == 0) {
                 tma_store_4d(&tmO, sO + s * 16384, s * 64, it.qb * BQ, it.h, it.b);
                 tma_store_commit();
