@@ -6,7 +6,7 @@
 One "step" = one pass of the hot path over one attention layer's inputs (BASELINE.json configs[1]:
 480p Wan-2.2-14B-shaped layer, H=40, N=32760, d=128, 25 % density block masks):
     chorus_mask_to_index (stored bitmask -> CSR)  ->  chorus_block_sparse_attn_fwd (BF16)
-    -> chorus_quantize_fp8 -> chorus_block_sparse_attn_fwd (FP8)         [FP8 leg when the build has it]
+    -> chorus_quantize_fp8 -> chorus_block_sparse_attn_fwd (FP8)         [--no-fp8 leaves this leg out]
 Metric: effective TFLOP/s on kept tiles, FLOPs = 4*N^2*d*H*density per attention call
 (BASELINE.json north_star).  Prints ONE JSON line (rank 0).
 
@@ -339,7 +339,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="chorus", choices=["chorus", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg4"])
-    ap.add_argument("--fp8", action="store_true", default=False)
+    ap.add_argument("--no-fp8", dest="fp8", action="store_false", default=True,
+                    help="leave the FP8 leg (quantise + FP8 attention) out of the step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "chorus" else args.warmup

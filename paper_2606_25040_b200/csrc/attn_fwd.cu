@@ -17,6 +17,11 @@
 // a row max grows by more than 2^8 over the reference that the accumulators currently use.  The
 // epilogue normalises, converts to bf16, stages in shared memory and writes with TMA stores
 // (coalesced 128-byte rows; rows beyond N are clipped by the tensor map).
+//
+// FP8 variant (template kFp8; R10-R12): e4m3 Q / K / V tiles (one 128-byte row holds all
+// 128 channels), tcgen05.mma kind::f8f6f4 with fp32 accumulation, V again an MN-major B operand,
+// P cast to e4m3 after a 2^5 shift, the Q / K block scales folded into the exp2 constant of each
+// 64-key tile and V's per-channel scale applied in the epilogue.
 #include <cuda_bf16.h>
 
 #include "chorus_internal.h"
@@ -28,36 +33,46 @@ namespace {
 using namespace ptx;
 
 constexpr int BQ = 128, BK = 64;
-constexpr int KSTAGES = 2, VSTAGES = 3, SBUFS = 3;
+constexpr int SBUFS = 3;
 constexpr int NUM_THREADS = 384;
 constexpr int PRODUCER_WARP = 8, MMA_WARP = 9;
 
-// shared memory map (bytes from a 1024-aligned base)
-constexpr uint32_t SQ_OFF = 0;                         // Q : 2 slabs [128 rows][128 B]      32 KB
-constexpr uint32_t SK_OFF = 32768;                     // K : KSTAGES x 2 slabs [128 keys][128 B]
-constexpr uint32_t SV_OFF = SK_OFF + KSTAGES * 32768;  // V : VSTAGES x 2 slabs [128 keys][128 B]
-constexpr uint32_t SO_OFF = SV_OFF + VSTAGES * 32768;  // O staging: 2 slabs [128 rows][128 B]
-constexpr uint32_t XCH_OFF = SO_OFF + 32768;           // row max / row sum exchange [2 parity][2 half][128] f32
-constexpr uint32_t BAR_OFF = XCH_OFF + 2048;
-constexpr uint32_t SMEM_BYTES = BAR_OFF + 256;
-static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
-
-// mbarrier slots (8 bytes each) from BAR_OFF
-enum : uint32_t {
-    B_Q_FULL = 0, B_Q_EMPTY = 1, B_K_FULL = 2, B_K_EMPTY = B_K_FULL + KSTAGES,
-    B_V_FULL = B_K_EMPTY + KSTAGES, B_V_EMPTY = B_V_FULL + VSTAGES, B_S_FULL = B_V_EMPTY + VSTAGES,
-    B_P_READY = B_S_FULL + SBUFS, B_PV_DONE = B_P_READY + SBUFS, B_O_FREE = B_PV_DONE + SBUFS,
-    B_COUNT = B_O_FREE + 1
+// Per-dtype geometry.  A "slab" is a [128 rows][128 B] swizzled tile: 64 bf16 channels or all 128
+// e4m3 channels of 128 rows (one Q block, or the two 64-key tiles of a pair).
+template <bool kFp8>
+struct Cfg {
+    static constexpr uint32_t SLABS = kFp8 ? 1 : 2;                 // slabs per 128-row, 128-channel tile
+    static constexpr uint32_t TILE_BYTES = SLABS * 16384;           // Q block, or one K / V pair stage
+    static constexpr uint32_t HALF_BYTES = 8192;                    // second tile of a pair inside a slab
+    static constexpr int KSTAGES = kFp8 ? 4 : 2, VSTAGES = kFp8 ? 4 : 3;
+    static constexpr uint32_t KSTEPS = kFp8 ? 4 : 8;                // MMAs per 128-deep contraction
+    // shared memory map (bytes from a 1024-aligned base)
+    static constexpr uint32_t SQ_OFF = 0;
+    static constexpr uint32_t SK_OFF = TILE_BYTES;
+    static constexpr uint32_t SV_OFF = SK_OFF + KSTAGES * TILE_BYTES;
+    static constexpr uint32_t SO_OFF = SV_OFF + VSTAGES * TILE_BYTES;   // O staging: 2 slabs (bf16 out)
+    static constexpr uint32_t XCH_OFF = SO_OFF + 32768;   // row max / sum exchange [2 parity][2 half][128] f32
+    static constexpr uint32_t BAR_OFF = XCH_OFF + 2048;
+    static constexpr uint32_t SMEM_BYTES = BAR_OFF + 256;
+    // mbarrier slots (8 bytes each) from BAR_OFF
+    static constexpr uint32_t B_Q_FULL = 0, B_Q_EMPTY = 1, B_K_FULL = 2, B_K_EMPTY = B_K_FULL + KSTAGES,
+        B_V_FULL = B_K_EMPTY + KSTAGES, B_V_EMPTY = B_V_FULL + VSTAGES, B_S_FULL = B_V_EMPTY + VSTAGES,
+        B_P_READY = B_S_FULL + SBUFS, B_PV_DONE = B_P_READY + SBUFS, B_O_FREE = B_PV_DONE + SBUFS,
+        B_COUNT = B_O_FREE + 1;
+    static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
+    static_assert(B_COUNT * 8 + 8 <= 256, "barrier area too small");
+    // P: exp2(x - m_ref + P_SHIFT).  bf16 keeps P <= 2^8 under the lazy threshold; e4m3 (max 448,
+    // smallest normal 2^-6) shifts P up by 2^5 and tightens the threshold to 2^3 so that P <= 2^8
+    // still holds while probabilities down to 2^-11 of the row maximum stay normal numbers.
+    static constexpr float RESCALE_THRESHOLD = kFp8 ? 3.0f : 8.0f;   // log2 units
+    static constexpr float P_SHIFT = kFp8 ? 5.0f : 0.0f;
 };
-static_assert(B_COUNT * 8 + 8 <= 256, "barrier area too small");
 
 // tensor-memory map (columns): three S buffers and the O accumulator
 constexpr uint32_t TM_S = 0, TM_O = 384, TM_COLS = 512;
 
 // named barriers: 0 = __syncthreads, 1..4 = warp pair (w, w+4), 5..6 = column-half warpgroup
 constexpr uint32_t NB_PAIR = 1, NB_HALF = 5;
-
-constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 units: p stays below 2^8
 
 __device__ __forceinline__ void setmaxnreg_inc_216() { asm volatile("setmaxnreg.inc.sync.aligned.u32 216;"); }
 __device__ __forceinline__ void setmaxnreg_dec_56() { asm volatile("setmaxnreg.dec.sync.aligned.u32 56;"); }
@@ -85,35 +100,38 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmO,
                 const AttnParams p) {
+    using C = Cfg<kFp8>;
+    constexpr int KSTAGES = C::KSTAGES, VSTAGES = C::VSTAGES;
+    constexpr uint32_t TILE = C::TILE_BYTES, HALF = C::HALF_BYTES;
     // 128-byte swizzle needs a 1024-byte aligned base; the kernel has no static shared memory, so
     // the dynamic window starts at the CTA's (1 KB granular) allocation.  Checked, not assumed.
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t base = smem_u32(smem_raw);
     if (base & 1023u) __trap();
     uint8_t* gbase = smem_raw;
-    const uint32_t sQ = base + SQ_OFF, sK = base + SK_OFF, sV = base + SV_OFF, sO = base + SO_OFF;
-    const uint32_t bars = base + BAR_OFF;
+    const uint32_t sQ = base + C::SQ_OFF, sK = base + C::SK_OFF, sV = base + C::SV_OFF, sO = base + C::SO_OFF;
+    const uint32_t bars = base + C::BAR_OFF;
     auto bar = [&](uint32_t i) { return bars + 8u * i; };
-    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gbase + BAR_OFF + 8 * B_COUNT);
-    volatile float* xch = reinterpret_cast<volatile float*>(gbase + XCH_OFF);
+    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gbase + C::BAR_OFF + 8 * C::B_COUNT);
+    volatile float* xch = reinterpret_cast<volatile float*>(gbase + C::XCH_OFF);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_items = p.B * p.H * p.nq;
 
     if (threadIdx.x == 0) {
-        mbar_init(bar(B_Q_FULL), 1);
-        mbar_init(bar(B_Q_EMPTY), 1);
-        for (int i = 0; i < KSTAGES; ++i) { mbar_init(bar(B_K_FULL + i), 1); mbar_init(bar(B_K_EMPTY + i), 1); }
-        for (int i = 0; i < VSTAGES; ++i) { mbar_init(bar(B_V_FULL + i), 1); mbar_init(bar(B_V_EMPTY + i), 1); }
+        mbar_init(bar(C::B_Q_FULL), 1);
+        mbar_init(bar(C::B_Q_EMPTY), 1);
+        for (int i = 0; i < KSTAGES; ++i) { mbar_init(bar(C::B_K_FULL + i), 1); mbar_init(bar(C::B_K_EMPTY + i), 1); }
+        for (int i = 0; i < VSTAGES; ++i) { mbar_init(bar(C::B_V_FULL + i), 1); mbar_init(bar(C::B_V_EMPTY + i), 1); }
         for (int i = 0; i < SBUFS; ++i) {
-            mbar_init(bar(B_S_FULL + i), 1);
-            mbar_init(bar(B_P_READY + i), 8);
-            mbar_init(bar(B_PV_DONE + i), 1);
+            mbar_init(bar(C::B_S_FULL + i), 1);
+            mbar_init(bar(C::B_P_READY + i), 8);
+            mbar_init(bar(C::B_PV_DONE + i), 1);
         }
-        mbar_init(bar(B_O_FREE), 8);
+        mbar_init(bar(C::B_O_FREE), 8);
         fence_mbar_init();
     }
-    if (warp == MMA_WARP) tmem_alloc(bars + 8 * B_COUNT, TM_COLS);
+    if (warp == MMA_WARP) tmem_alloc(bars + 8 * C::B_COUNT, TM_COLS);
     if (warp == PRODUCER_WARP && lane == 0) {
         prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV); prefetch_tmap(&tmO);
     }
@@ -126,49 +144,47 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // ======================= producer / MMA warpgroup ==========================================
         setmaxnreg_dec_56();
         if (warp == PRODUCER_WARP && lane == 0) {
+            // one 128-row, 128-channel box = SLABS loads of [rows][128 B]
+            auto load_tile = [&](uint32_t dst, const CUtensorMap* tm, uint32_t b, int row0, int h, int bb) {
+                tma_load_4d(dst, tm, b, 0, row0, h, bb);
+                if constexpr (!kFp8) tma_load_4d(dst + 16384, tm, b, 64, row0, h, bb);
+            };
             uint32_t g = 0, icnt = 0;   // pairs and non-empty items issued so far
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
                 const Item it = get_item(p, idx);
                 if (it.nt == 0) continue;   // empty rows touch no barrier
-                mbar_wait(bar(B_Q_EMPTY), (icnt & 1) ^ 1);
-                mbar_arrive_expect_tx(bar(B_Q_FULL), 32768);
-                tma_load_4d(sQ, &tmQ, bar(B_Q_FULL), 0, it.qb * BQ, it.h, it.b);
-                tma_load_4d(sQ + 16384, &tmQ, bar(B_Q_FULL), 64, it.qb * BQ, it.h, it.b);
+                mbar_wait(bar(C::B_Q_EMPTY), (icnt & 1) ^ 1);
+                mbar_arrive_expect_tx(bar(C::B_Q_FULL), TILE);
+                load_tile(sQ, &tmQ, bar(C::B_Q_FULL), it.qb * BQ, it.h, it.b);
                 for (int j = 0; j < it.np; ++j, ++g) {
                     const int ntile = (2 * j + 1 < it.nt) ? 2 : 1;
                     const int kb0 = __ldg(p.col_idx + it.r0 + 2 * j);
                     const int kb1 = (ntile == 2) ? __ldg(p.col_idx + it.r0 + 2 * j + 1) : 0;
                     {
                         const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1;
-                        mbar_wait(bar(B_K_EMPTY + st), ph ^ 1);
-                        mbar_arrive_expect_tx(bar(B_K_FULL + st), ntile * 16384);
-                        const uint32_t dst = sK + st * 32768;
-                        tma_load_4d(dst, &tmK, bar(B_K_FULL + st), 0, kb0 * BK, it.h, it.b);
-                        tma_load_4d(dst + 16384, &tmK, bar(B_K_FULL + st), 64, kb0 * BK, it.h, it.b);
-                        if (ntile == 2) {
-                            tma_load_4d(dst + 8192, &tmK, bar(B_K_FULL + st), 0, kb1 * BK, it.h, it.b);
-                            tma_load_4d(dst + 16384 + 8192, &tmK, bar(B_K_FULL + st), 64, kb1 * BK, it.h, it.b);
-                        }
+                        mbar_wait(bar(C::B_K_EMPTY + st), ph ^ 1);
+                        mbar_arrive_expect_tx(bar(C::B_K_FULL + st), ntile * (TILE / 2));
+                        const uint32_t dst = sK + st * TILE;
+                        load_tile(dst, &tmK, bar(C::B_K_FULL + st), kb0 * BK, it.h, it.b);
+                        if (ntile == 2) load_tile(dst + HALF, &tmK, bar(C::B_K_FULL + st), kb1 * BK, it.h, it.b);
                     }
                     {
                         const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1;
-                        mbar_wait(bar(B_V_EMPTY + st), ph ^ 1);
-                        mbar_arrive_expect_tx(bar(B_V_FULL + st), ntile * 16384);
-                        const uint32_t dst = sV + st * 32768;
-                        tma_load_4d(dst, &tmV, bar(B_V_FULL + st), 0, kb0 * BK, it.h, it.b);
-                        tma_load_4d(dst + 16384, &tmV, bar(B_V_FULL + st), 64, kb0 * BK, it.h, it.b);
-                        if (ntile == 2) {
-                            tma_load_4d(dst + 8192, &tmV, bar(B_V_FULL + st), 0, kb1 * BK, it.h, it.b);
-                            tma_load_4d(dst + 16384 + 8192, &tmV, bar(B_V_FULL + st), 64, kb1 * BK, it.h, it.b);
-                        }
+                        mbar_wait(bar(C::B_V_EMPTY + st), ph ^ 1);
+                        mbar_arrive_expect_tx(bar(C::B_V_FULL + st), ntile * (TILE / 2));
+                        const uint32_t dst = sV + st * TILE;
+                        load_tile(dst, &tmV, bar(C::B_V_FULL + st), kb0 * BK, it.h, it.b);
+                        if (ntile == 2) load_tile(dst + HALF, &tmV, bar(C::B_V_FULL + st), kb1 * BK, it.h, it.b);
                     }
                 }
                 ++icnt;
             }
         } else if (warp == MMA_WARP && lane == 0) {
-            constexpr uint32_t IDESC_S128 = make_idesc(1, 1, 128, 128, 0, 0);
-            constexpr uint32_t IDESC_S64 = make_idesc(1, 1, 128, 64, 0, 0);
-            constexpr uint32_t IDESC_PV = make_idesc(1, 1, 128, 128, 0, 1);
+            // kind::f16: format 1 = bf16; kind::f8f6f4: format 0 = e4m3.  PV: B (= V) is MN-major.
+            constexpr uint32_t FMT = kFp8 ? 0u : 1u;
+            constexpr uint32_t IDESC_S128 = make_idesc(FMT, FMT, 128, 128, 0, 0);
+            constexpr uint32_t IDESC_S64 = make_idesc(FMT, FMT, 128, 64, 0, 0);
+            constexpr uint32_t IDESC_PV = make_idesc(FMT, FMT, 128, 128, 0, 1);
             const uint64_t dQ = smem_desc_sw128(sQ, 16, 1024);
             const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
             const uint64_t dV = smem_desc_sw128(sV, 16384, 1024);
@@ -176,47 +192,64 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
                 const Item it = get_item(p, idx);
                 if (it.nt == 0) continue;
-                mbar_wait(bar(B_Q_FULL), icnt & 1);
+                mbar_wait(bar(C::B_Q_FULL), icnt & 1);
                 for (int jj = 0; jj < it.np + 2; ++jj) {
                     if (jj < it.np) {   // S[g % 3] = Q K^T of pair jj (runs up to two pairs ahead)
                         const uint32_t g = g0 + jj;
                         const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1, sb = g % SBUFS;
                         const int ntile = (2 * jj + 1 < it.nt) ? 2 : 1;
-                        mbar_wait(bar(B_K_FULL + st), ph);
+                        mbar_wait(bar(C::B_K_FULL + st), ph);
                         tc_fence_after();
                         const uint32_t tS = tmem + TM_S + sb * 128;
                         const uint32_t idesc = (ntile == 2) ? IDESC_S128 : IDESC_S64;
-                        const uint64_t dKs = dK + ((st * 32768u) >> 4);
+                        const uint64_t dKs = dK + ((st * TILE) >> 4);
+                        if constexpr (kFp8) {
 #pragma unroll
-                        for (int ks = 0; ks < 8; ++ks) {
-                            const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
-                            mma_f16_ss(tS, dQ + off, dKs + off, idesc, ks > 0);
+                            for (int ks = 0; ks < 4; ++ks)       // 32 e4m3 channels = 32 B per step
+                                mma_f8_ss(tS, dQ + ((ks * 32) >> 4), dKs + ((ks * 32) >> 4), idesc, ks > 0);
+                        } else {
+#pragma unroll
+                            for (int ks = 0; ks < 8; ++ks) {     // 16 bf16 channels = 32 B per step, 2 slabs
+                                const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
+                                mma_f16_ss(tS, dQ + off, dKs + off, idesc, ks > 0);
+                            }
                         }
-                        tc_commit(bar(B_K_EMPTY + st));
-                        tc_commit(bar(B_S_FULL + sb));
-                        if (jj == it.np - 1) tc_commit(bar(B_Q_EMPTY));
+                        tc_commit(bar(C::B_K_EMPTY + st));
+                        tc_commit(bar(C::B_S_FULL + sb));
+                        if (jj == it.np - 1) tc_commit(bar(C::B_Q_EMPTY));
                     }
                     if (jj >= 2) {      // O += P V of pair jj - 2
                         const int jp = jj - 2;
                         const uint32_t g = g0 + jp;
                         const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1, sb = g % SBUFS;
                         const int ntile = (2 * jp + 1 < it.nt) ? 2 : 1;
-                        mbar_wait(bar(B_P_READY + sb), (g / SBUFS) & 1);
-                        mbar_wait(bar(B_V_FULL + st), ph);
-                        if (jp == 0) mbar_wait(bar(B_O_FREE), (icnt & 1) ^ 1);
+                        mbar_wait(bar(C::B_P_READY + sb), (g / SBUFS) & 1);
+                        mbar_wait(bar(C::B_V_FULL + st), ph);
+                        if (jp == 0) mbar_wait(bar(C::B_O_FREE), (icnt & 1) ^ 1);
                         tc_fence_after();
                         const uint32_t tP = tmem + TM_S + sb * 128, tO = tmem + TM_O;
-                        const uint64_t dVs = dV + ((st * 32768u) >> 4);
+                        const uint64_t dVs = dV + ((st * TILE) >> 4);
+                        if constexpr (kFp8) {
 #pragma unroll
-                        for (int ks = 0; ks < 8; ++ks) {
-                            if (ks < 4 * ntile) {
-                                // P of tile 0 lives in S columns [0, 32), P of tile 1 in [64, 96)
-                                const uint32_t ta = tP + (ks >> 2) * 64 + (ks & 3) * 8;
-                                mma_f16_ts(tO, ta, dVs + ((ks * 2048u) >> 4), IDESC_PV, (jp > 0) || (ks > 0));
+                            for (int ks = 0; ks < 4; ++ks) {     // 32 keys per step: 8 TMEM columns of e4m3 P
+                                if (ks < 2 * ntile) {
+                                    // P of tile 0 lives in S columns [0, 16), P of tile 1 in [64, 80)
+                                    const uint32_t ta = tP + (ks >> 1) * 64 + (ks & 1) * 8;
+                                    mma_f8_ts(tO, ta, dVs + ((ks * 4096u) >> 4), IDESC_PV, (jp > 0) || (ks > 0));
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int ks = 0; ks < 8; ++ks) {     // 16 keys per step: 8 TMEM columns of bf16 P
+                                if (ks < 4 * ntile) {
+                                    // P of tile 0 lives in S columns [0, 32), P of tile 1 in [64, 96)
+                                    const uint32_t ta = tP + (ks >> 2) * 64 + (ks & 3) * 8;
+                                    mma_f16_ts(tO, ta, dVs + ((ks * 2048u) >> 4), IDESC_PV, (jp > 0) || (ks > 0));
+                                }
                             }
                         }
-                        tc_commit(bar(B_V_EMPTY + st));
-                        tc_commit(bar(B_PV_DONE + sb));
+                        tc_commit(bar(C::B_V_EMPTY + st));
+                        tc_commit(bar(C::B_PV_DONE + sb));
                     }
                 }
                 g0 += it.np;
@@ -231,21 +264,44 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int row = wq * 32 + lane;          // query row inside the block == TMEM lane
         const uint32_t tlane = tmem + (static_cast<uint32_t>(wq * 32) << 16);
         const uint32_t tO = tlane + TM_O + s * 64;   // this warp rescales / finalises O columns [64 s, 64 s + 64)
-        const float sl2 = p.scale_log2;
+        const int nsb = (p.N + 127) >> 7;        // FP8: Q/K scale blocks of 128 tokens
         uint32_t g = 0;                          // pairs processed so far (all items)
         uint32_t xc = 0;                         // exchanges so far: slot parity (two slots, one barrier each)
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
             const Item it = get_item(p, idx);
             float m_ref = -INFINITY, l0 = 0.f, l1 = 0.f;
+            // FP8 (R10): scores are (q8 . k8) * s_q[qb] * s_k[kb / 2]; the per-tile factor is
+            // folded into the exp2 FMA constant.  kb (and its scale) of the NEXT pair are fetched
+            // one pair ahead so that the loads are off the critical path.
+            float sl2 = p.scale_log2;
+            float qsl2 = 0.f;
+            const float* ksc = nullptr;
+            int kb_next = 0;
+            if constexpr (kFp8) {
+                const int64_t sbase = (static_cast<int64_t>(it.b) * p.H + it.h) * nsb;
+                qsl2 = p.scale_log2 * __ldg(p.q_scale + sbase + it.qb);
+                ksc = p.k_scale + sbase;
+                if (s < it.nt) kb_next = __ldg(p.col_idx + it.r0 + s);
+            }
             for (int j = 0; j < it.np; ++j, ++g) {
                 const uint32_t sb = g % SBUFS;
                 const uint32_t tS = tlane + TM_S + sb * 128 + s * 64;
                 int valid = BK;                  // valid keys in this warp's tile of the pair
-                if (j == it.np - 1) {            // only the last pair can be odd or hold the ragged key block
-                    if (2 * j + s < it.nt) valid = min(BK, p.N - __ldg(p.col_idx + it.r0 + 2 * j + s) * BK);
-                    else valid = 0;
+                int kb = 0;
+                if constexpr (kFp8) {
+                    kb = kb_next;
+                    if (2 * (j + 1) + s < it.nt) kb_next = __ldg(p.col_idx + it.r0 + 2 * (j + 1) + s);
+                    sl2 = qsl2 * __ldg(ksc + (kb >> 1));
                 }
-                mbar_wait(bar(B_S_FULL + sb), (g / SBUFS) & 1);
+                if (j == it.np - 1) {            // only the last pair can be odd or hold the ragged key block
+                    if (2 * j + s < it.nt) {
+                        if constexpr (!kFp8) kb = __ldg(p.col_idx + it.r0 + 2 * j + s);
+                        valid = min(BK, p.N - kb * BK);
+                    } else {
+                        valid = 0;
+                    }
+                }
+                mbar_wait(bar(C::B_S_FULL + sb), (g / SBUFS) & 1);
                 tc_fence_after();
                 uint32_t sv[64];
                 float mx = -INFINITY;
@@ -266,14 +322,14 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         a2 = max3(a2, __uint_as_float(sv[k + 4]), __uint_as_float(sv[k + 5]));
                         a3 = max3(a3, __uint_as_float(sv[k + 6]), __uint_as_float(sv[k + 7]));
                     }
-                    mx = fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)) * sl2;
+                    mx = fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)) * sl2;   // sl2 > 0
                 }
                 // the row max of the pair: exchange with the warp that holds the other 64 columns
                 const uint32_t par = (xc++) & 1;
                 xch[(par * 2 + s) * 128 + row] = mx;
                 named_bar_sync(NB_PAIR + wq, 64);
                 const float mt = fmaxf(mx, xch[(par * 2 + (s ^ 1)) * 128 + row]);
-                if (__any_sync(0xffffffffu, mt > m_ref + RESCALE_THRESHOLD)) {
+                if (__any_sync(0xffffffffu, mt > m_ref + C::RESCALE_THRESHOLD)) {
                     // identical decision in both warps of the pair (same mt, same m_ref per row)
                     const float m_new = fmaxf(m_ref, mt);
                     const float alpha = ex2(m_ref - m_new);   // m_ref = -inf (first pair) -> 0
@@ -284,7 +340,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         // O holds pairs 0..j-1 under the old reference; wait for P V of pair j-1.
                         // (S_FULL of pair g implies P V of pair g-3 is complete, so the barrier of
                         // buffer (g-1) % 3 is at most one phase behind: the parity wait is exact.)
-                        mbar_wait(bar(B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
+                        mbar_wait(bar(C::B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
                         tc_fence_after();
 #pragma unroll 1
                         for (int c = 0; c < 2; ++c) {
@@ -298,25 +354,47 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     }
                 }
                 if (valid > 0) {
-                    const float neg_m = -m_ref;
+                    const float neg_m = C::P_SHIFT - m_ref;
+                    if constexpr (kFp8) {
+                        // The denominator sums the e4m3-ROUNDED weights (two f16x2 accumulators per
+                        // 32 keys: at most 8 x 2^8 each, exact to 2^-11), i.e. exactly what P V uses.
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        uint32_t pk[8];
+                        for (int c = 0; c < 2; ++c) {            // 32 keys -> 8 columns of 4 e4m3 each
+                            uint32_t pk[8];
+                            uint32_t h0 = 0u, h1 = 0u;
 #pragma unroll
-                        for (int k = 0; k < 8; ++k) {
-                            const float p0 = ex2(fmaf(__uint_as_float(sv[c * 16 + 2 * k]), sl2, neg_m));
-                            const float p1 = ex2(fmaf(__uint_as_float(sv[c * 16 + 2 * k + 1]), sl2, neg_m));
-                            l0 += p0;
-                            l1 += p1;
-                            pk[k] = pack_bf16x2(p0, p1);
+                            for (int k = 0; k < 8; ++k) {
+                                const int e = c * 32 + 4 * k;
+                                const float p0 = ex2(fmaf(__uint_as_float(sv[e]), sl2, neg_m));
+                                const float p1 = ex2(fmaf(__uint_as_float(sv[e + 1]), sl2, neg_m));
+                                const float p2 = ex2(fmaf(__uint_as_float(sv[e + 2]), sl2, neg_m));
+                                const float p3 = ex2(fmaf(__uint_as_float(sv[e + 3]), sl2, neg_m));
+                                pk[k] = pack_e4m3x4_acc(p0, p1, p2, p3, h0, h1);
+                            }
+                            l0 += f16x2_hsum(h0);
+                            l1 += f16x2_hsum(h1);
+                            tmem_st8(tS + c * 8, pk);   // P: e4m3 quads over this warp's first 16 S columns
                         }
-                        tmem_st8(tS + c * 8, pk);   // P: bf16 pairs over this warp's first 32 S columns
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            uint32_t pk[8];
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) {
+                                const float p0 = ex2(fmaf(__uint_as_float(sv[c * 16 + 2 * k]), sl2, neg_m));
+                                const float p1 = ex2(fmaf(__uint_as_float(sv[c * 16 + 2 * k + 1]), sl2, neg_m));
+                                l0 += p0;
+                                l1 += p1;
+                                pk[k] = pack_bf16x2(p0, p1);
+                            }
+                            tmem_st8(tS + c * 8, pk);   // P: bf16 pairs over this warp's first 32 S columns
+                        }
                     }
                 }
                 tc_wait_st();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_P_READY + sb));
+                if (lane == 0) mbar_arrive(bar(C::B_P_READY + sb));
             }
             // ---------------- epilogue: normalise, convert, store --------------------------------
             const float l = l0 + l1;
@@ -328,10 +406,14 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const float inv = (L > 0.f) ? 1.f / L : 0.f;
             named_bar_sync(NB_HALF + s, 128);                  // staging free for the whole warpgroup
             if (it.nt > 0) {
-                mbar_wait(bar(B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
+                mbar_wait(bar(C::B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
                 tc_fence_after();
             }
             const uint32_t srow = sO + s * 16384 + row * 128;
+            // FP8: O[:, c] carries V's per-channel scale (R10)
+            const float4* vsc = nullptr;
+            if constexpr (kFp8)
+                vsc = reinterpret_cast<const float4*>(p.v_scale + (static_cast<int64_t>(it.b) * p.H + it.h) * 128 + s * 64);
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
                 uint32_t o[32];
@@ -341,10 +423,19 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 }
                 uint32_t pk[16];
 #pragma unroll
-                for (int k = 0; k < 16; ++k) {
-                    float x0 = 0.f, x1 = 0.f;
-                    if (it.nt > 0) { x0 = __uint_as_float(o[2 * k]) * inv; x1 = __uint_as_float(o[2 * k + 1]) * inv; }
-                    pk[k] = pack_bf16x2(x0, x1);
+                for (int k4 = 0; k4 < 8; ++k4) {
+                    float4 w = make_float4(inv, inv, inv, inv);
+                    if constexpr (kFp8) {
+                        const float4 sc = __ldg(vsc + c * 8 + k4);
+                        w = make_float4(inv * sc.x, inv * sc.y, inv * sc.z, inv * sc.w);
+                    }
+                    float x0 = 0.f, x1 = 0.f, x2 = 0.f, x3 = 0.f;
+                    if (it.nt > 0) {
+                        x0 = __uint_as_float(o[4 * k4]) * w.x;     x1 = __uint_as_float(o[4 * k4 + 1]) * w.y;
+                        x2 = __uint_as_float(o[4 * k4 + 2]) * w.z; x3 = __uint_as_float(o[4 * k4 + 3]) * w.w;
+                    }
+                    pk[2 * k4] = pack_bf16x2(x0, x1);
+                    pk[2 * k4 + 1] = pack_bf16x2(x2, x3);
                 }
 #pragma unroll
                 for (int q4 = 0; q4 < 4; ++q4) {
@@ -357,7 +448,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             if (it.nt > 0) {
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_O_FREE));
+                if (lane == 0) mbar_arrive(bar(C::B_O_FREE));
             }
             fence_proxy_async_smem();
             named_bar_sync(NB_HALF + s, 128);
@@ -375,21 +466,28 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 }  // namespace
 
-cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
-                            const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
-                            cudaStream_t stream) {
-    if (dtype != CHORUS_BF16) return cudaErrorNotSupported;
-    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+template <bool kFp8>
+static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
+                              const CUtensorMap& tmO, const AttnParams& p, cudaStream_t stream) {
+    constexpr uint32_t smem = Cfg<kFp8>::SMEM_BYTES;
+    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kFp8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     const int n_items = p.B * p.H * p.nq;
     const int grid = n_items < sms ? n_items : sms;
-    attn_fwd_kernel<false><<<grid, NUM_THREADS, SMEM_BYTES, stream>>>(tmQ, tmK, tmV, tmO, p);
+    attn_fwd_kernel<kFp8><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
     count_launch(1);
     return cudaGetLastError();
+}
+
+cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
+                            const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
+                            cudaStream_t stream) {
+    if (dtype == CHORUS_BF16) return launch_one<false>(tmQ, tmK, tmV, tmO, p, stream);
+    if (dtype == CHORUS_FP8_E4M3) return launch_one<true>(tmQ, tmK, tmV, tmO, p, stream);
+    return cudaErrorNotSupported;
 }
 
 }  // namespace chorus
