@@ -32,6 +32,9 @@ namespace {
 
 using namespace ptx;
 
+#ifndef CHORUS_POLY_MASK
+#define CHORUS_POLY_MASK 0x00u   // e.g. 0x4A = 3 of every 8 element pairs
+#endif
 constexpr int BQ = 128, BK = 64;
 constexpr int SBUFS = 3;
 constexpr int NUM_THREADS = 384;
@@ -66,6 +69,10 @@ struct Cfg {
     // still holds while probabilities down to 2^-11 of the row maximum stay normal numbers.
     static constexpr float RESCALE_THRESHOLD = kFp8 ? 3.0f : 8.0f;   // log2 units
     static constexpr float P_SHIFT = kFp8 ? 5.0f : 0.0f;
+    // which element pairs (index mod 8) take the FMA-pipe polynomial exp2 instead of the MUFU, and
+    // its degree (relative error 7.5e-5 / 1.7e-3, below the bf16 / e4m3 rounding of P)
+    static constexpr uint32_t POLY_MASK = CHORUS_POLY_MASK;
+    static constexpr int POLY_DEG = kFp8 ? 2 : 3;
 };
 
 // tensor-memory map (columns): three S buffers and the O accumulator
@@ -354,7 +361,17 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     }
                 }
                 if (valid > 0) {
-                    const float neg_m = C::P_SHIFT - m_ref;
+                    // P = exp2(s * sl2 - m_ref + shift).  Element pairs go through packed FFMA2; the
+                    // pairs whose bit is set in POLY_MASK (index mod 8) take the polynomial exp2 on
+                    // the FMA pipe, the rest the MUFU, so that both pipes finish together.
+                    const float2 sl2_2 = make_float2(sl2, sl2);
+                    const float2 negm_2 = make_float2(C::P_SHIFT - m_ref, C::P_SHIFT - m_ref);
+                    auto exp_pair = [&](int q) -> float2 {     // q: element pair index 0..31
+                        const float2 x = ffma2(make_float2(__uint_as_float(sv[2 * q]), __uint_as_float(sv[2 * q + 1])),
+                                               sl2_2, negm_2);
+                        if ((C::POLY_MASK >> (q & 7)) & 1u) return exp2_poly2<C::POLY_DEG>(x);
+                        return make_float2(ex2(x.x), ex2(x.y));
+                    };
                     if constexpr (kFp8) {
                         // The denominator sums the e4m3-ROUNDED weights (two f16x2 accumulators per
                         // 32 keys: at most 8 x 2^8 each, exact to 2^-11), i.e. exactly what P V uses.
@@ -364,31 +381,28 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             uint32_t h0 = 0u, h1 = 0u;
 #pragma unroll
                             for (int k = 0; k < 8; ++k) {
-                                const int e = c * 32 + 4 * k;
-                                const float p0 = ex2(fmaf(__uint_as_float(sv[e]), sl2, neg_m));
-                                const float p1 = ex2(fmaf(__uint_as_float(sv[e + 1]), sl2, neg_m));
-                                const float p2 = ex2(fmaf(__uint_as_float(sv[e + 2]), sl2, neg_m));
-                                const float p3 = ex2(fmaf(__uint_as_float(sv[e + 3]), sl2, neg_m));
-                                pk[k] = pack_e4m3x4_acc(p0, p1, p2, p3, h0, h1);
+                                const float2 pa = exp_pair(c * 16 + 2 * k), pb = exp_pair(c * 16 + 2 * k + 1);
+                                pk[k] = pack_e4m3x4_acc(pa.x, pa.y, pb.x, pb.y, h0, h1);
                             }
                             l0 += f16x2_hsum(h0);
                             l1 += f16x2_hsum(h1);
                             tmem_st8(tS + c * 8, pk);   // P: e4m3 quads over this warp's first 16 S columns
                         }
                     } else {
+                        float2 lacc = make_float2(l0, l1);
 #pragma unroll
                         for (int c = 0; c < 4; ++c) {
                             uint32_t pk[8];
 #pragma unroll
                             for (int k = 0; k < 8; ++k) {
-                                const float p0 = ex2(fmaf(__uint_as_float(sv[c * 16 + 2 * k]), sl2, neg_m));
-                                const float p1 = ex2(fmaf(__uint_as_float(sv[c * 16 + 2 * k + 1]), sl2, neg_m));
-                                l0 += p0;
-                                l1 += p1;
-                                pk[k] = pack_bf16x2(p0, p1);
+                                const float2 pp = exp_pair(c * 8 + k);
+                                lacc = fadd2(lacc, pp);
+                                pk[k] = pack_bf16x2(pp.x, pp.y);
                             }
                             tmem_st8(tS + c * 8, pk);   // P: bf16 pairs over this warp's first 32 S columns
                         }
+                        l0 = lacc.x;
+                        l1 = lacc.y;
                     }
                 }
                 tc_wait_st();
