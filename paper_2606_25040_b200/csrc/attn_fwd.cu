@@ -1,21 +1,25 @@
 // attn_fwd.cu — chorus_block_sparse_attn_fwd for sm_100a ("skip pruned block pairs and
 // evaluate only the retained ones in QK^T, softmax, and PV").
 //
-// Persistent, warp-specialised kernel, one CTA (384 threads) per SM:
-//   warp 8        TMA producer: Q tile once per work item, then the kept K / V tiles of the CSR row,
-//                 two 64-key tiles ("a pair") per pipeline stage, 128-byte swizzle
-//   warp 9        MMA issuer (one thread): S = Q K^T (M=128, N=128, K=128) into one of THREE S
-//                 buffers in tensor memory, up to two pairs ahead of the softmax; O += P V
-//                 (M=128, N=128, K=128) with P as the TMEM A operand and V as an MN-major
-//                 shared-memory B operand
-//   warps 0-7     softmax.  Warp w owns TMEM lanes 32*(w%4).. (one query row per thread) and the
-//                 64 score columns of tile (w/4) of the pair: warps w and w+4 share their rows'
-//                 running max through shared memory and a 64-thread named barrier per pair.
-// A work item is one (batch, head, 128-row query block).  Its kept tiles are paired (any two kept
-// tiles, not necessarily adjacent keys) so that QK^T runs at N=128.  P (bf16) overwrites the first
-// half of each warp's own S columns.  O (fp32, 128 columns of TMEM) is rescaled lazily: only when
-// a row max grows by more than 2^8 over the reference that the accumulators currently use.  The
-// epilogue normalises, converts to bf16, stages in shared memory and writes with TMA stores
+// Persistent, warp-specialised kernel, one CTA (384 threads) per SM.  A work item is one (batch,
+// head, 128-row query block).  Its kept 64-key tiles are taken two at a time ("a pair": any two kept
+// tiles, not necessarily adjacent keys) so that QK^T runs at N=128, and the pairs are dealt
+// alternately to two independent STREAMS (even pairs / odd pairs), each with its own S buffer, its
+// own O accumulator in tensor memory and its own running max / sum:
+//   warp 8        TMA producer: Q tile once per item, then the K / V tiles of every pair into two
+//                 rings, 128-byte swizzle
+//   warp 9        MMA issuer (one thread): S_st = Q K^T (M=128, N=128, K=128) and O_st += P_st V
+//                 (P the TMEM A operand, V an MN-major shared-memory B operand), issued in the order
+//                 S(0) S(1) PV(0) S(2) PV(1) S(3) ... so that one stream's softmax overlaps the other
+//                 stream's MMAs
+//   warps 0-3     softmax of stream 0; warps 4-7 softmax of stream 1.  Warp w owns TMEM lanes
+//                 32*(w%4).. (one query row per thread) and all 128 score columns of its pair, so
+//                 the main loop has no cross-warp exchange at all; the two warps of an SM
+//                 sub-partition (w, w+4) work on different pairs and keep its MUFU busy in turn.
+// P (bf16 / e4m3) overwrites the first columns of its S buffer.  Each O (fp32, 128 TMEM columns) is
+// rescaled lazily: only when a row max grows by more than 2^8 (2^3 for FP8) over the reference its
+// accumulator uses.  The epilogue merges the two streams (O = (a0 O0 + a1 O1) / (a0 l0 + a1 l1),
+// a_st = 2^(m_st - max m)), converts to bf16, stages in shared memory and writes with TMA stores
 // (coalesced 128-byte rows; rows beyond N are clipped by the tensor map).
 //
 // FP8 variant (template kFp8; R10-R12): e4m3 Q / K / V tiles (one 128-byte row holds all
@@ -36,7 +40,6 @@ using namespace ptx;
 #define CHORUS_POLY_MASK 0x00u   // e.g. 0x4A = 3 of every 8 element pairs
 #endif
 constexpr int BQ = 128, BK = 64;
-constexpr int SBUFS = 3;
 constexpr int NUM_THREADS = 384;
 constexpr int PRODUCER_WARP = 8, MMA_WARP = 9;
 
@@ -48,19 +51,18 @@ struct Cfg {
     static constexpr uint32_t TILE_BYTES = SLABS * 16384;           // Q block, or one K / V pair stage
     static constexpr uint32_t HALF_BYTES = 8192;                    // second tile of a pair inside a slab
     static constexpr int KSTAGES = kFp8 ? 4 : 2, VSTAGES = kFp8 ? 4 : 3;
-    static constexpr uint32_t KSTEPS = kFp8 ? 4 : 8;                // MMAs per 128-deep contraction
     // shared memory map (bytes from a 1024-aligned base)
     static constexpr uint32_t SQ_OFF = 0;
     static constexpr uint32_t SK_OFF = TILE_BYTES;
     static constexpr uint32_t SV_OFF = SK_OFF + KSTAGES * TILE_BYTES;
     static constexpr uint32_t SO_OFF = SV_OFF + VSTAGES * TILE_BYTES;   // O staging: 2 slabs (bf16 out)
-    static constexpr uint32_t XCH_OFF = SO_OFF + 32768;   // row max / sum exchange [2 parity][2 half][128] f32
+    static constexpr uint32_t XCH_OFF = SO_OFF + 32768;   // epilogue exchange [2 stream][m, l][128] f32
     static constexpr uint32_t BAR_OFF = XCH_OFF + 2048;
     static constexpr uint32_t SMEM_BYTES = BAR_OFF + 256;
     // mbarrier slots (8 bytes each) from BAR_OFF
     static constexpr uint32_t B_Q_FULL = 0, B_Q_EMPTY = 1, B_K_FULL = 2, B_K_EMPTY = B_K_FULL + KSTAGES,
         B_V_FULL = B_K_EMPTY + KSTAGES, B_V_EMPTY = B_V_FULL + VSTAGES, B_S_FULL = B_V_EMPTY + VSTAGES,
-        B_P_READY = B_S_FULL + SBUFS, B_PV_DONE = B_P_READY + SBUFS, B_O_FREE = B_PV_DONE + SBUFS,
+        B_P_READY = B_S_FULL + 2, B_ITEM_DONE = B_P_READY + 2, B_O_FREE = B_ITEM_DONE + 1,
         B_COUNT = B_O_FREE + 1;
     static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
     static_assert(B_COUNT * 8 + 8 <= 256, "barrier area too small");
@@ -73,10 +75,12 @@ struct Cfg {
     // its degree (relative error 7.5e-5 / 1.7e-3, below the bf16 / e4m3 rounding of P)
     static constexpr uint32_t POLY_MASK = CHORUS_POLY_MASK;
     static constexpr int POLY_DEG = kFp8 ? 2 : 3;
+    // TMEM columns of P per MMA step (16 bf16 keys or 32 e4m3 keys = 8 columns), steps per tile
+    static constexpr int PV_STEPS_PER_TILE = kFp8 ? 2 : 4;
 };
 
-// tensor-memory map (columns): three S buffers and the O accumulator
-constexpr uint32_t TM_S = 0, TM_O = 384, TM_COLS = 512;
+// tensor-memory map (columns): S (aliased by P) and O of stream 0, then of stream 1
+constexpr uint32_t TM_S = 0, TM_O = 256, TM_COLS = 512;   // S_st = TM_S + 128 st, O_st = TM_O + 128 st
 
 // named barriers: 0 = __syncthreads, 1..4 = warp pair (w, w+4), 5..6 = column-half warpgroup
 constexpr uint32_t NB_PAIR = 1, NB_HALF = 5;
@@ -101,6 +105,19 @@ __device__ __forceinline__ Item get_item(const AttnParams& p, int idx) {
 }
 
 __device__ __forceinline__ float max3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
+
+// max of 64 fp32 bit patterns
+__device__ __forceinline__ float max64(const uint32_t* sv) {
+    float a0 = -INFINITY, a1 = -INFINITY, a2 = -INFINITY, a3 = -INFINITY;
+#pragma unroll
+    for (int k = 0; k < 64; k += 8) {
+        a0 = max3(a0, __uint_as_float(sv[k]), __uint_as_float(sv[k + 1]));
+        a1 = max3(a1, __uint_as_float(sv[k + 2]), __uint_as_float(sv[k + 3]));
+        a2 = max3(a2, __uint_as_float(sv[k + 4]), __uint_as_float(sv[k + 5]));
+        a3 = max3(a3, __uint_as_float(sv[k + 6]), __uint_as_float(sv[k + 7]));
+    }
+    return fmaxf(fmaxf(a0, a1), fmaxf(a2, a3));
+}
 
 template <bool kFp8>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
@@ -130,11 +147,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(bar(C::B_Q_EMPTY), 1);
         for (int i = 0; i < KSTAGES; ++i) { mbar_init(bar(C::B_K_FULL + i), 1); mbar_init(bar(C::B_K_EMPTY + i), 1); }
         for (int i = 0; i < VSTAGES; ++i) { mbar_init(bar(C::B_V_FULL + i), 1); mbar_init(bar(C::B_V_EMPTY + i), 1); }
-        for (int i = 0; i < SBUFS; ++i) {
+        for (int i = 0; i < 2; ++i) {
             mbar_init(bar(C::B_S_FULL + i), 1);
-            mbar_init(bar(C::B_P_READY + i), 8);
-            mbar_init(bar(C::B_PV_DONE + i), 1);
+            mbar_init(bar(C::B_P_READY + i), 4);
         }
+        mbar_init(bar(C::B_ITEM_DONE), 1);
         mbar_init(bar(C::B_O_FREE), 8);
         fence_mbar_init();
     }
@@ -195,19 +212,21 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const uint64_t dQ = smem_desc_sw128(sQ, 16, 1024);
             const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
             const uint64_t dV = smem_desc_sw128(sV, 16384, 1024);
-            uint32_t g0 = 0, icnt = 0;   // pairs before this item, non-empty items so far
+            uint32_t g0 = 0, icnt = 0;      // pairs before this item, non-empty items so far
+            uint32_t cnt[2] = {0u, 0u};     // P V products issued per stream (phase of P_READY)
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
                 const Item it = get_item(p, idx);
                 if (it.nt == 0) continue;
                 mbar_wait(bar(C::B_Q_FULL), icnt & 1);
-                for (int jj = 0; jj < it.np + 2; ++jj) {
-                    if (jj < it.np) {   // S[g % 3] = Q K^T of pair jj (runs up to two pairs ahead)
+                for (int jj = 0; jj <= it.np; ++jj) {
+                    if (jj < it.np) {   // S_st = Q K^T of pair jj, stream st = jj & 1.  Its buffer is free:
+                                        // P V of pair jj - 2 was issued before (in-order tensor pipe).
                         const uint32_t g = g0 + jj;
-                        const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1, sb = g % SBUFS;
+                        const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1, sm = jj & 1;
                         const int ntile = (2 * jj + 1 < it.nt) ? 2 : 1;
                         mbar_wait(bar(C::B_K_FULL + st), ph);
                         tc_fence_after();
-                        const uint32_t tS = tmem + TM_S + sb * 128;
+                        const uint32_t tS = tmem + TM_S + sm * 128;
                         const uint32_t idesc = (ntile == 2) ? IDESC_S128 : IDESC_S64;
                         const uint64_t dKs = dK + ((st * TILE) >> 4);
                         if constexpr (kFp8) {
@@ -222,41 +241,33 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             }
                         }
                         tc_commit(bar(C::B_K_EMPTY + st));
-                        tc_commit(bar(C::B_S_FULL + sb));
+                        tc_commit(bar(C::B_S_FULL + sm));
                         if (jj == it.np - 1) tc_commit(bar(C::B_Q_EMPTY));
                     }
-                    if (jj >= 2) {      // O += P V of pair jj - 2
-                        const int jp = jj - 2;
+                    if (jj >= 1) {      // O_st += P V of pair jj - 1
+                        const int jp = jj - 1;
                         const uint32_t g = g0 + jp;
-                        const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1, sb = g % SBUFS;
+                        const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1, sm = jp & 1;
                         const int ntile = (2 * jp + 1 < it.nt) ? 2 : 1;
-                        mbar_wait(bar(C::B_P_READY + sb), (g / SBUFS) & 1);
+                        mbar_wait(bar(C::B_P_READY + sm), cnt[sm] & 1);
+                        ++cnt[sm];
                         mbar_wait(bar(C::B_V_FULL + st), ph);
                         if (jp == 0) mbar_wait(bar(C::B_O_FREE), (icnt & 1) ^ 1);
                         tc_fence_after();
-                        const uint32_t tP = tmem + TM_S + sb * 128, tO = tmem + TM_O;
+                        const uint32_t tP = tmem + TM_S + sm * 128, tO = tmem + TM_O + sm * 128;
                         const uint64_t dVs = dV + ((st * TILE) >> 4);
-                        if constexpr (kFp8) {
+                        constexpr uint32_t KBYTES = kFp8 ? 4096u : 2048u;   // 32 / 16 keys x 128 B per step
 #pragma unroll
-                            for (int ks = 0; ks < 4; ++ks) {     // 32 keys per step: 8 TMEM columns of e4m3 P
-                                if (ks < 2 * ntile) {
-                                    // P of tile 0 lives in S columns [0, 16), P of tile 1 in [64, 80)
-                                    const uint32_t ta = tP + (ks >> 1) * 64 + (ks & 1) * 8;
-                                    mma_f8_ts(tO, ta, dVs + ((ks * 4096u) >> 4), IDESC_PV, (jp > 0) || (ks > 0));
-                                }
-                            }
-                        } else {
-#pragma unroll
-                            for (int ks = 0; ks < 8; ++ks) {     // 16 keys per step: 8 TMEM columns of bf16 P
-                                if (ks < 4 * ntile) {
-                                    // P of tile 0 lives in S columns [0, 32), P of tile 1 in [64, 96)
-                                    const uint32_t ta = tP + (ks >> 2) * 64 + (ks & 3) * 8;
-                                    mma_f16_ts(tO, ta, dVs + ((ks * 2048u) >> 4), IDESC_PV, (jp > 0) || (ks > 0));
-                                }
+                        for (int ks = 0; ks < 2 * C::PV_STEPS_PER_TILE; ++ks) {
+                            if (ks < C::PV_STEPS_PER_TILE * ntile) {
+                                // the stream's first pair (jp = 0 or 1) starts its accumulator afresh
+                                const uint32_t acc = (jp > 1) || (ks > 0);
+                                if constexpr (kFp8) mma_f8_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
+                                else mma_f16_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
                             }
                         }
                         tc_commit(bar(C::B_V_EMPTY + st));
-                        tc_commit(bar(C::B_PV_DONE + sb));
+                        if (jp == it.np - 1) tc_commit(bar(C::B_ITEM_DONE));
                     }
                 }
                 g0 += it.np;
@@ -266,190 +277,228 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     } else {
         // ======================= softmax warps ======================================================
         setmaxnreg_inc_216();
-        const int s = warp >> 2;                 // which tile of the pair: score columns [64 s, 64 s + 64)
+        const int sm = warp >> 2;                // stream: pairs sm, sm + 2, ... of every item
         const int wq = warp & 3;                 // TMEM lane quarter
         const int row = wq * 32 + lane;          // query row inside the block == TMEM lane
         const uint32_t tlane = tmem + (static_cast<uint32_t>(wq * 32) << 16);
-        const uint32_t tO = tlane + TM_O + s * 64;   // this warp rescales / finalises O columns [64 s, 64 s + 64)
+        const uint32_t tS = tlane + TM_S + sm * 128;          // this stream's S / P
+        const uint32_t tOs = tlane + TM_O + sm * 128;         // this stream's O accumulator
         const int nsb = (p.N + 127) >> 7;        // FP8: Q/K scale blocks of 128 tokens
-        uint32_t g = 0;                          // pairs processed so far (all items)
-        uint32_t xc = 0;                         // exchanges so far: slot parity (two slots, one barrier each)
+        uint32_t cnt = 0;                        // pairs this stream has processed (phase of S_FULL)
+        uint32_t icnt = 0;                       // non-empty items so far
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
             const Item it = get_item(p, idx);
             float m_ref = -INFINITY, l0 = 0.f, l1 = 0.f;
             // FP8 (R10): scores are (q8 . k8) * s_q[qb] * s_k[kb / 2]; the per-tile factor is
-            // folded into the exp2 FMA constant.  kb (and its scale) of the NEXT pair are fetched
-            // one pair ahead so that the loads are off the critical path.
-            float sl2 = p.scale_log2;
+            // folded into the exp2 FMA constant.  The key-block indices of the stream's NEXT pair are
+            // fetched one pair ahead so that the loads are off the critical path.
+            float sl2a = p.scale_log2, sl2b = p.scale_log2;
             float qsl2 = 0.f;
             const float* ksc = nullptr;
-            int kb_next = 0;
+            int kba_next = 0, kbb_next = 0;
             if constexpr (kFp8) {
                 const int64_t sbase = (static_cast<int64_t>(it.b) * p.H + it.h) * nsb;
                 qsl2 = p.scale_log2 * __ldg(p.q_scale + sbase + it.qb);
                 ksc = p.k_scale + sbase;
-                if (s < it.nt) kb_next = __ldg(p.col_idx + it.r0 + s);
+                if (2 * sm < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * sm);
+                if (2 * sm + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * sm + 1);
             }
-            for (int j = 0; j < it.np; ++j, ++g) {
-                const uint32_t sb = g % SBUFS;
-                const uint32_t tS = tlane + TM_S + sb * 128 + s * 64;
-                int valid = BK;                  // valid keys in this warp's tile of the pair
-                int kb = 0;
+            for (int j = sm; j < it.np; j += 2, ++cnt) {
+                int va = BK, vb = BK;            // valid keys in the two tiles of the pair
+                int kba = 0, kbb = 0;
                 if constexpr (kFp8) {
-                    kb = kb_next;
-                    if (2 * (j + 1) + s < it.nt) kb_next = __ldg(p.col_idx + it.r0 + 2 * (j + 1) + s);
-                    sl2 = qsl2 * __ldg(ksc + (kb >> 1));
+                    kba = kba_next;
+                    kbb = kbb_next;
+                    if (2 * (j + 2) < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2));
+                    if (2 * (j + 2) + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2) + 1);
+                    sl2a = qsl2 * __ldg(ksc + (kba >> 1));
+                    sl2b = qsl2 * __ldg(ksc + (kbb >> 1));
                 }
                 if (j == it.np - 1) {            // only the last pair can be odd or hold the ragged key block
-                    if (2 * j + s < it.nt) {
-                        if constexpr (!kFp8) kb = __ldg(p.col_idx + it.r0 + 2 * j + s);
-                        valid = min(BK, p.N - kb * BK);
-                    } else {
-                        valid = 0;
+                    if constexpr (!kFp8) {
+                        kba = __ldg(p.col_idx + it.r0 + 2 * j);
+                        if (2 * j + 1 < it.nt) kbb = __ldg(p.col_idx + it.r0 + 2 * j + 1);
                     }
+                    va = min(BK, p.N - kba * BK);
+                    vb = (2 * j + 1 < it.nt) ? min(BK, p.N - kbb * BK) : 0;
                 }
-                mbar_wait(bar(C::B_S_FULL + sb), (g / SBUFS) & 1);
+                mbar_wait(bar(C::B_S_FULL + sm), cnt & 1);
                 tc_fence_after();
-                uint32_t sv[64];
-                float mx = -INFINITY;
-                if (valid > 0) {
-                    tmem_ld32(tS, *reinterpret_cast<uint32_t(*)[32]>(sv));
-                    tmem_ld32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(sv + 32));
+                // The 128 scores of a row are streamed from tensor memory twice, 32 columns at a time
+                // with the next chunk's load in flight (pass 1: row max; pass 2: exp, pack, store P
+                // behind the read position), so that only 64 of them are ever live in registers.
+                const bool ragged = (va < BK) || (vb < BK);   // warp-uniform, last pair of a row only
+                auto mask_chunk = [&](uint32_t (&r)[32], int c) {
+                    const int valid = ((c >> 1) ? vb : va) - 32 * (c & 1);
+#pragma unroll
+                    for (int k = 0; k < 32; ++k)
+                        if (k >= valid) r[k] = 0xff800000u;   // -inf
+                };
+                auto max32 = [](const uint32_t (&r)[32]) {
+                    float a0 = -INFINITY, a1 = -INFINITY;
+#pragma unroll
+                    for (int k = 0; k < 32; k += 4) {
+                        a0 = max3(a0, __uint_as_float(r[k]), __uint_as_float(r[k + 1]));
+                        a1 = max3(a1, __uint_as_float(r[k + 2]), __uint_as_float(r[k + 3]));
+                    }
+                    return fmaxf(a0, a1);
+                };
+                uint32_t ra[32], rb[32];
+                float mxa, mxb;
+                {
+                    tmem_ld32(tS, ra);
                     tc_wait_ld();
-                    if (valid < BK) {
-#pragma unroll
-                        for (int k = 0; k < 64; ++k)
-                            if (k >= valid) sv[k] = 0xff800000u;   // -inf
-                    }
-                    float a0 = -INFINITY, a1 = -INFINITY, a2 = -INFINITY, a3 = -INFINITY;
-#pragma unroll
-                    for (int k = 0; k < 64; k += 8) {
-                        a0 = max3(a0, __uint_as_float(sv[k]), __uint_as_float(sv[k + 1]));
-                        a1 = max3(a1, __uint_as_float(sv[k + 2]), __uint_as_float(sv[k + 3]));
-                        a2 = max3(a2, __uint_as_float(sv[k + 4]), __uint_as_float(sv[k + 5]));
-                        a3 = max3(a3, __uint_as_float(sv[k + 6]), __uint_as_float(sv[k + 7]));
-                    }
-                    mx = fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)) * sl2;   // sl2 > 0
+                    tmem_ld32(tS + 32, rb);
+                    if (ragged) mask_chunk(ra, 0);
+                    mxa = max32(ra);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 64, ra);
+                    if (ragged) mask_chunk(rb, 1);
+                    mxa = fmaxf(mxa, max32(rb));
+                    tc_wait_ld();
+                    tmem_ld32(tS + 96, rb);
+                    if (ragged) mask_chunk(ra, 2);
+                    mxb = max32(ra);
+                    tc_wait_ld();
+                    tmem_ld32(tS, ra);                       // first chunk of pass 2
+                    if (ragged) mask_chunk(rb, 3);
+                    mxb = fmaxf(mxb, max32(rb));
                 }
-                // the row max of the pair: exchange with the warp that holds the other 64 columns
-                const uint32_t par = (xc++) & 1;
-                xch[(par * 2 + s) * 128 + row] = mx;
-                named_bar_sync(NB_PAIR + wq, 64);
-                const float mt = fmaxf(mx, xch[(par * 2 + (s ^ 1)) * 128 + row]);
+                const float mt = fmaxf(mxa * sl2a, mxb * sl2b);   // sl2 > 0; va > 0
                 if (__any_sync(0xffffffffu, mt > m_ref + C::RESCALE_THRESHOLD)) {
-                    // identical decision in both warps of the pair (same mt, same m_ref per row)
                     const float m_new = fmaxf(m_ref, mt);
                     const float alpha = ex2(m_ref - m_new);   // m_ref = -inf (first pair) -> 0
                     l0 *= alpha;
                     l1 *= alpha;
                     m_ref = m_new;
-                    if (j > 0) {
-                        // O holds pairs 0..j-1 under the old reference; wait for P V of pair j-1.
-                        // (S_FULL of pair g implies P V of pair g-3 is complete, so the barrier of
-                        // buffer (g-1) % 3 is at most one phase behind: the parity wait is exact.)
-                        mbar_wait(bar(C::B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
-                        tc_fence_after();
+                    if (j >= 2) {
+                        // O_st holds this stream's earlier pairs under the old reference.  S_FULL of
+                        // pair j was committed after P V of pair j - 2 on the in-order tensor pipe,
+                        // so that product is complete and nothing else touches O_st until P_READY.
 #pragma unroll 1
-                        for (int c = 0; c < 2; ++c) {
-                            uint32_t o[32];
-                            tmem_ld32(tO + c * 32, o);
+                        for (int c = 0; c < 4; ++c) {
+                            tc_wait_ld();
+                            tmem_ld32(tOs + c * 32, rb);
                             tc_wait_ld();
 #pragma unroll
-                            for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * alpha);
-                            tmem_st32(tO + c * 32, o);
+                            for (int k = 0; k < 32; ++k) rb[k] = __float_as_uint(__uint_as_float(rb[k]) * alpha);
+                            tmem_st32(tOs + c * 32, rb);
                         }
                     }
                 }
-                if (valid > 0) {
+                {
                     // P = exp2(s * sl2 - m_ref + shift).  Element pairs go through packed FFMA2; the
                     // pairs whose bit is set in POLY_MASK (index mod 8) take the polynomial exp2 on
-                    // the FMA pipe, the rest the MUFU, so that both pipes finish together.
-                    const float2 sl2_2 = make_float2(sl2, sl2);
+                    // the FMA pipe, the rest the MUFU.
                     const float2 negm_2 = make_float2(C::P_SHIFT - m_ref, C::P_SHIFT - m_ref);
-                    auto exp_pair = [&](int q) -> float2 {     // q: element pair index 0..31
-                        const float2 x = ffma2(make_float2(__uint_as_float(sv[2 * q]), __uint_as_float(sv[2 * q + 1])),
-                                               sl2_2, negm_2);
-                        if ((C::POLY_MASK >> (q & 7)) & 1u) return exp2_poly2<C::POLY_DEG>(x);
-                        return make_float2(ex2(x.x), ex2(x.y));
-                    };
-                    if constexpr (kFp8) {
-                        // The denominator sums the e4m3-ROUNDED weights (two f16x2 accumulators per
-                        // 32 keys: at most 8 x 2^8 each, exact to 2^-11), i.e. exactly what P V uses.
-#pragma unroll
-                        for (int c = 0; c < 2; ++c) {            // 32 keys -> 8 columns of 4 e4m3 each
+                    const float2 sl2a_2 = make_float2(sl2a, sl2a), sl2b_2 = make_float2(sl2b, sl2b);
+                    float2 lacc = make_float2(l0, l1);
+                    // 32 scores -> 16 (bf16) / 8 (e4m3) TMEM columns of P at chunk position c
+                    auto exp_chunk = [&](const uint32_t (&r)[32], int c) {
+                        const float2 sl2_2 = (c >> 1) ? sl2b_2 : sl2a_2;
+                        auto exp_pair = [&](int q) -> float2 {     // q: element pair index 0..15
+                            const float2 x = ffma2(make_float2(__uint_as_float(r[2 * q]), __uint_as_float(r[2 * q + 1])),
+                                                   sl2_2, negm_2);
+                            if ((C::POLY_MASK >> (q & 7)) & 1u) return exp2_poly2<C::POLY_DEG>(x);
+                            return make_float2(ex2(x.x), ex2(x.y));
+                        };
+                        if constexpr (kFp8) {
+                            // The denominator sums the e4m3-ROUNDED weights (two f16x2 accumulators
+                            // per 32 keys: at most 8 x 2^8 each, exact to 2^-11): exactly what P V uses.
                             uint32_t pk[8];
                             uint32_t h0 = 0u, h1 = 0u;
 #pragma unroll
                             for (int k = 0; k < 8; ++k) {
-                                const float2 pa = exp_pair(c * 16 + 2 * k), pb = exp_pair(c * 16 + 2 * k + 1);
+                                const float2 pa = exp_pair(2 * k), pb = exp_pair(2 * k + 1);
                                 pk[k] = pack_e4m3x4_acc(pa.x, pa.y, pb.x, pb.y, h0, h1);
                             }
-                            l0 += f16x2_hsum(h0);
-                            l1 += f16x2_hsum(h1);
-                            tmem_st8(tS + c * 8, pk);   // P: e4m3 quads over this warp's first 16 S columns
-                        }
-                    } else {
-                        float2 lacc = make_float2(l0, l1);
+                            lacc.x += f16x2_hsum(h0);
+                            lacc.y += f16x2_hsum(h1);
+                            tmem_st8(tS + c * 8, pk);        // P: e4m3 quads over the first 32 S columns
+                        } else {
+                            uint32_t pk[16];
 #pragma unroll
-                        for (int c = 0; c < 4; ++c) {
-                            uint32_t pk[8];
-#pragma unroll
-                            for (int k = 0; k < 8; ++k) {
-                                const float2 pp = exp_pair(c * 8 + k);
+                            for (int k = 0; k < 16; ++k) {
+                                const float2 pp = exp_pair(k);
                                 lacc = fadd2(lacc, pp);
                                 pk[k] = pack_bf16x2(pp.x, pp.y);
                             }
-                            tmem_st8(tS + c * 8, pk);   // P: bf16 pairs over this warp's first 32 S columns
+                            tmem_st16(tS + c * 16, pk);      // P: bf16 pairs over the first 64 S columns
                         }
-                        l0 = lacc.x;
-                        l1 = lacc.y;
-                    }
+                    };
+                    tc_wait_ld();
+                    tmem_ld32(tS + 32, rb);
+                    if (ragged) mask_chunk(ra, 0);
+                    exp_chunk(ra, 0);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 64, ra);
+                    if (ragged) mask_chunk(rb, 1);
+                    exp_chunk(rb, 1);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 96, rb);
+                    if (ragged) mask_chunk(ra, 2);
+                    exp_chunk(ra, 2);
+                    tc_wait_ld();
+                    if (ragged) mask_chunk(rb, 3);
+                    exp_chunk(rb, 3);
+                    l0 = lacc.x;
+                    l1 = lacc.y;
                 }
                 tc_wait_st();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(C::B_P_READY + sb));
+                if (lane == 0) mbar_arrive(bar(C::B_P_READY + sm));
             }
-            // ---------------- epilogue: normalise, convert, store --------------------------------
-            const float l = l0 + l1;
-            const uint32_t par = (xc++) & 1;
-            xch[(par * 2 + s) * 128 + row] = l;
-            if (lane == 0 && wq == 0) tma_store_wait_read();   // staging slab s is free again
+            // ---------------- epilogue: merge the two streams, normalise, convert, store ----------
+            // Warp (sm, wq) finalises O columns [64 sm, 64 sm + 64) of its 32 rows from BOTH accumulators.
+            const float l_mine = l0 + l1;
+            xch[(sm * 2 + 0) * 128 + row] = m_ref;
+            xch[(sm * 2 + 1) * 128 + row] = l_mine;
+            if (lane == 0 && wq == 0) tma_store_wait_read();   // staging slab sm is free again
             named_bar_sync(NB_PAIR + wq, 64);
-            const float L = l + xch[(par * 2 + (s ^ 1)) * 128 + row];
+            const float m_oth = xch[((sm ^ 1) * 2 + 0) * 128 + row];
+            const float l_oth = xch[((sm ^ 1) * 2 + 1) * 128 + row];
+            named_bar_sync(NB_PAIR + wq, 64);                  // both have read: the slots may be rewritten
+            const float m_all = fmaxf(m_ref, m_oth);
+            // a stream without pairs has m = -inf, l = 0: weight 0 and its accumulator is not read
+            const float a_mine = (m_ref == -INFINITY) ? 0.f : ex2(m_ref - m_all);
+            const float a_oth = (m_oth == -INFINITY) ? 0.f : ex2(m_oth - m_all);
+            const float L = l_mine * a_mine + l_oth * a_oth;
             const float inv = (L > 0.f) ? 1.f / L : 0.f;
-            named_bar_sync(NB_HALF + s, 128);                  // staging free for the whole warpgroup
+            const float w0 = (sm == 0 ? a_mine : a_oth) * inv, w1 = (sm == 0 ? a_oth : a_mine) * inv;
+            named_bar_sync(NB_HALF + sm, 128);                 // staging free for the whole warpgroup
             if (it.nt > 0) {
-                mbar_wait(bar(C::B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
+                mbar_wait(bar(C::B_ITEM_DONE), icnt & 1);      // every P V of the item has completed
                 tc_fence_after();
             }
-            const uint32_t srow = sO + s * 16384 + row * 128;
+            const uint32_t srow = sO + sm * 16384 + row * 128;
+            const uint32_t tO0 = tlane + TM_O + sm * 64, tO1 = tlane + TM_O + 128 + sm * 64;
             // FP8: O[:, c] carries V's per-channel scale (R10)
             const float4* vsc = nullptr;
             if constexpr (kFp8)
-                vsc = reinterpret_cast<const float4*>(p.v_scale + (static_cast<int64_t>(it.b) * p.H + it.h) * 128 + s * 64);
+                vsc = reinterpret_cast<const float4*>(p.v_scale + (static_cast<int64_t>(it.b) * p.H + it.h) * 128 + sm * 64);
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
-                uint32_t o[32];
-                if (it.nt > 0) {
-                    tmem_ld32(tO + c * 32, o);
-                    tc_wait_ld();
-                }
+                uint32_t o0[32], o1[32];
+                const bool has0 = it.nt > 0, has1 = it.np > 1;     // warp-uniform
+                if (has0) tmem_ld32(tO0 + c * 32, o0);
+                if (has1) tmem_ld32(tO1 + c * 32, o1);
+                if (has0) tc_wait_ld();
                 uint32_t pk[16];
 #pragma unroll
                 for (int k4 = 0; k4 < 8; ++k4) {
-                    float4 w = make_float4(inv, inv, inv, inv);
-                    if constexpr (kFp8) {
-                        const float4 sc = __ldg(vsc + c * 8 + k4);
-                        w = make_float4(inv * sc.x, inv * sc.y, inv * sc.z, inv * sc.w);
+                    float4 sc = make_float4(1.f, 1.f, 1.f, 1.f);
+                    if constexpr (kFp8) sc = __ldg(vsc + c * 8 + k4);
+                    float x[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        float v = 0.f;
+                        if (has0) v = __uint_as_float(o0[4 * k4 + e]) * w0;
+                        if (has1) v = fmaf(__uint_as_float(o1[4 * k4 + e]), w1, v);
+                        x[e] = v;
                     }
-                    float x0 = 0.f, x1 = 0.f, x2 = 0.f, x3 = 0.f;
-                    if (it.nt > 0) {
-                        x0 = __uint_as_float(o[4 * k4]) * w.x;     x1 = __uint_as_float(o[4 * k4 + 1]) * w.y;
-                        x2 = __uint_as_float(o[4 * k4 + 2]) * w.z; x3 = __uint_as_float(o[4 * k4 + 3]) * w.w;
-                    }
-                    pk[2 * k4] = pack_bf16x2(x0, x1);
-                    pk[2 * k4 + 1] = pack_bf16x2(x2, x3);
+                    pk[2 * k4] = pack_bf16x2(x[0] * sc.x, x[1] * sc.y);
+                    pk[2 * k4 + 1] = pack_bf16x2(x[2] * sc.z, x[3] * sc.w);
                 }
 #pragma unroll
                 for (int q4 = 0; q4 < 4; ++q4) {
@@ -463,11 +512,12 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(C::B_O_FREE));
+                ++icnt;
             }
             fence_proxy_async_smem();
-            named_bar_sync(NB_HALF + s, 128);
+            named_bar_sync(NB_HALF + sm, 128);
             if (lane == 0 && wq == 0) {
-                tma_store_4d(&tmO, sO + s * 16384, s * 64, it.qb * BQ, it.h, it.b);
+                tma_store_4d(&tmO, sO + sm * 16384, sm * 64, it.qb * BQ, it.h, it.b);
                 tma_store_commit();
             }
         }
