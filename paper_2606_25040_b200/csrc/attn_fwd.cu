@@ -3,23 +3,24 @@
 //
 // Persistent, warp-specialised kernel, one CTA (384 threads) per SM.  A work item is one (batch,
 // head, 128-row query block).  Its kept 64-key tiles are taken two at a time ("a pair": any two kept
-// tiles, not necessarily adjacent keys) so that QK^T runs at N=128, and the pairs are dealt
-// alternately to two independent STREAMS (even pairs / odd pairs), each with its own S buffer, its
-// own O accumulator in tensor memory and its own running max / sum:
+// tiles, not necessarily adjacent keys) so that QK^T runs at N=128.
 //   warp 8        TMA producer: Q tile once per item, then the K / V tiles of every pair into two
 //                 rings, 128-byte swizzle
-//   warp 9        MMA issuer (one thread): S_st = Q K^T (M=128, N=128, K=128) and O_st += P_st V
-//                 (P the TMEM A operand, V an MN-major shared-memory B operand), issued in the order
-//                 S(0) S(1) PV(0) S(2) PV(1) S(3) ... so that one stream's softmax overlaps the other
-//                 stream's MMAs
-//   warps 0-3     softmax of stream 0; warps 4-7 softmax of stream 1.  Warp w owns TMEM lanes
-//                 32*(w%4).. (one query row per thread) and all 128 score columns of its pair, so
-//                 the main loop has no cross-warp exchange at all; the two warps of an SM
-//                 sub-partition (w, w+4) work on different pairs and keep its MUFU busy in turn.
-// P (bf16 / e4m3) overwrites the first columns of its S buffer.  Each O (fp32, 128 TMEM columns) is
-// rescaled lazily: only when a row max grows by more than 2^8 (2^3 for FP8) over the reference its
-// accumulator uses.  The epilogue merges the two streams (O = (a0 O0 + a1 O1) / (a0 l0 + a1 l1),
-// a_st = 2^(m_st - max m)), converts to bf16, stages in shared memory and writes with TMA stores
+//   warp 9        MMA issuer (one thread): S = Q K^T (M=128, N=128, K=128) into one of THREE S buffers
+//                 in tensor memory, up to two pairs ahead of the softmax; O += P V (P the TMEM A
+//                 operand, V an MN-major shared-memory B operand) into ONE accumulator
+//   warps 0-3     softmax of the even pairs of an item; warps 4-7 of the odd pairs.  Warp w owns TMEM
+//                 lanes 32*(w%4).. (one query row per thread) and all 128 score columns of its
+//                 pair.  The two warps of an SM sub-partition (w, w+4) therefore work on
+//                 consecutive pairs, half a period apart: one's exp phase (MUFU) overlaps the
+//                 other's load / max phase.  They share one running reference m_ref per row, handed
+//                 from pair j to pair j+1 through shared memory and a 64-thread named barrier
+//                 (arrive after the max pass of pair j, sync before the exp pass of pair j+1).
+// The 128 scores of a row are streamed from tensor memory twice, 32 columns at a time (max pass,
+// then exp pass), so only 64 are live in registers.  P (bf16 / e4m3) overwrites the first columns of
+// its S buffer behind the read position.  O (fp32, 128 TMEM columns) is rescaled lazily: only when a
+// row max grows by more than 2^8 (2^3 for FP8) over m_ref.  The epilogue adds the two warps' partial
+// row sums, normalises, converts to bf16, stages in shared memory and writes with TMA stores
 // (coalesced 128-byte rows; rows beyond N are clipped by the tensor map).
 //
 // FP8 variant (template kFp8; R10-R12): e4m3 Q / K / V tiles (one 128-byte row holds all
@@ -40,6 +41,7 @@ using namespace ptx;
 #define CHORUS_POLY_MASK 0x00u   // e.g. 0x4A = 3 of every 8 element pairs
 #endif
 constexpr int BQ = 128, BK = 64;
+constexpr int SBUFS = 3;
 constexpr int NUM_THREADS = 384;
 constexpr int PRODUCER_WARP = 8, MMA_WARP = 9;
 
@@ -56,14 +58,14 @@ struct Cfg {
     static constexpr uint32_t SK_OFF = TILE_BYTES;
     static constexpr uint32_t SV_OFF = SK_OFF + KSTAGES * TILE_BYTES;
     static constexpr uint32_t SO_OFF = SV_OFF + VSTAGES * TILE_BYTES;   // O staging: 2 slabs (bf16 out)
-    static constexpr uint32_t XCH_OFF = SO_OFF + 32768;   // epilogue exchange [2 stream][m, l][128] f32
-    static constexpr uint32_t BAR_OFF = XCH_OFF + 2048;
+    static constexpr uint32_t XCH_OFF = SO_OFF + 32768;   // f32 [128] m_ref hand-off, [2][2][128] epilogue (m, l)
+    static constexpr uint32_t BAR_OFF = XCH_OFF + 2560;
     static constexpr uint32_t SMEM_BYTES = BAR_OFF + 256;
     // mbarrier slots (8 bytes each) from BAR_OFF
     static constexpr uint32_t B_Q_FULL = 0, B_Q_EMPTY = 1, B_K_FULL = 2, B_K_EMPTY = B_K_FULL + KSTAGES,
         B_V_FULL = B_K_EMPTY + KSTAGES, B_V_EMPTY = B_V_FULL + VSTAGES, B_S_FULL = B_V_EMPTY + VSTAGES,
-        B_P_READY = B_S_FULL + 2, B_ITEM_DONE = B_P_READY + 2, B_O_FREE = B_ITEM_DONE + 1,
-        B_COUNT = B_O_FREE + 1;
+        B_P_READY = B_S_FULL + SBUFS, B_PV_DONE = B_P_READY + SBUFS, B_ITEM_DONE = B_PV_DONE + SBUFS,
+        B_O_FREE = B_ITEM_DONE + 1, B_COUNT = B_O_FREE + 1;
     static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
     static_assert(B_COUNT * 8 + 8 <= 256, "barrier area too small");
     // P: exp2(x - m_ref + P_SHIFT).  bf16 keeps P <= 2^8 under the lazy threshold; e4m3 (max 448,
@@ -79,11 +81,12 @@ struct Cfg {
     static constexpr int PV_STEPS_PER_TILE = kFp8 ? 2 : 4;
 };
 
-// tensor-memory map (columns): S (aliased by P) and O of stream 0, then of stream 1
-constexpr uint32_t TM_S = 0, TM_O = 256, TM_COLS = 512;   // S_st = TM_S + 128 st, O_st = TM_O + 128 st
+// tensor-memory map (columns): three S buffers (each aliased by its P) and the O accumulator
+constexpr uint32_t TM_S = 0, TM_O = 384, TM_COLS = 512;
 
-// named barriers: 0 = __syncthreads, 1..4 = warp pair (w, w+4), 5..6 = column-half warpgroup
-constexpr uint32_t NB_PAIR = 1, NB_HALF = 5;
+// named barriers: 0 = __syncthreads, 1..4 = warp pair (w, w+4) in the epilogue, 5..6 = column-half
+// warpgroup, 7..14 = m_ref hand-off published by parity 0 (7..10) / parity 1 (11..14) of quarter wq
+constexpr uint32_t NB_PAIR = 1, NB_HALF = 5, NB_HAND = 7;
 
 __device__ __forceinline__ void setmaxnreg_inc_216() { asm volatile("setmaxnreg.inc.sync.aligned.u32 216;"); }
 __device__ __forceinline__ void setmaxnreg_dec_56() { asm volatile("setmaxnreg.dec.sync.aligned.u32 56;"); }
@@ -147,9 +150,10 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(bar(C::B_Q_EMPTY), 1);
         for (int i = 0; i < KSTAGES; ++i) { mbar_init(bar(C::B_K_FULL + i), 1); mbar_init(bar(C::B_K_EMPTY + i), 1); }
         for (int i = 0; i < VSTAGES; ++i) { mbar_init(bar(C::B_V_FULL + i), 1); mbar_init(bar(C::B_V_EMPTY + i), 1); }
-        for (int i = 0; i < 2; ++i) {
+        for (int i = 0; i < SBUFS; ++i) {
             mbar_init(bar(C::B_S_FULL + i), 1);
             mbar_init(bar(C::B_P_READY + i), 4);
+            mbar_init(bar(C::B_PV_DONE + i), 1);
         }
         mbar_init(bar(C::B_ITEM_DONE), 1);
         mbar_init(bar(C::B_O_FREE), 8);
@@ -213,20 +217,18 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
             const uint64_t dV = smem_desc_sw128(sV, 16384, 1024);
             uint32_t g0 = 0, icnt = 0;      // pairs before this item, non-empty items so far
-            uint32_t cnt[2] = {0u, 0u};     // P V products issued per stream (phase of P_READY)
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
                 const Item it = get_item(p, idx);
                 if (it.nt == 0) continue;
                 mbar_wait(bar(C::B_Q_FULL), icnt & 1);
-                for (int jj = 0; jj <= it.np; ++jj) {
-                    if (jj < it.np) {   // S_st = Q K^T of pair jj, stream st = jj & 1.  Its buffer is free:
-                                        // P V of pair jj - 2 was issued before (in-order tensor pipe).
+                for (int jj = 0; jj < it.np + 2; ++jj) {
+                    if (jj < it.np) {   // S[g % 3] = Q K^T of pair jj (runs up to two pairs ahead)
                         const uint32_t g = g0 + jj;
-                        const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1, sm = jj & 1;
+                        const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1, sb = g % SBUFS;
                         const int ntile = (2 * jj + 1 < it.nt) ? 2 : 1;
                         mbar_wait(bar(C::B_K_FULL + st), ph);
                         tc_fence_after();
-                        const uint32_t tS = tmem + TM_S + sm * 128;
+                        const uint32_t tS = tmem + TM_S + sb * 128;
                         const uint32_t idesc = (ntile == 2) ? IDESC_S128 : IDESC_S64;
                         const uint64_t dKs = dK + ((st * TILE) >> 4);
                         if constexpr (kFp8) {
@@ -241,32 +243,31 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             }
                         }
                         tc_commit(bar(C::B_K_EMPTY + st));
-                        tc_commit(bar(C::B_S_FULL + sm));
+                        tc_commit(bar(C::B_S_FULL + sb));
                         if (jj == it.np - 1) tc_commit(bar(C::B_Q_EMPTY));
                     }
-                    if (jj >= 1) {      // O_st += P V of pair jj - 1
-                        const int jp = jj - 1;
+                    if (jj >= 2) {      // O += P V of pair jj - 2
+                        const int jp = jj - 2;
                         const uint32_t g = g0 + jp;
-                        const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1, sm = jp & 1;
+                        const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1, sb = g % SBUFS;
                         const int ntile = (2 * jp + 1 < it.nt) ? 2 : 1;
-                        mbar_wait(bar(C::B_P_READY + sm), cnt[sm] & 1);
-                        ++cnt[sm];
+                        mbar_wait(bar(C::B_P_READY + sb), (g / SBUFS) & 1);
                         mbar_wait(bar(C::B_V_FULL + st), ph);
                         if (jp == 0) mbar_wait(bar(C::B_O_FREE), (icnt & 1) ^ 1);
                         tc_fence_after();
-                        const uint32_t tP = tmem + TM_S + sm * 128, tO = tmem + TM_O + sm * 128;
+                        const uint32_t tP = tmem + TM_S + sb * 128, tO = tmem + TM_O;
                         const uint64_t dVs = dV + ((st * TILE) >> 4);
                         constexpr uint32_t KBYTES = kFp8 ? 4096u : 2048u;   // 32 / 16 keys x 128 B per step
 #pragma unroll
                         for (int ks = 0; ks < 2 * C::PV_STEPS_PER_TILE; ++ks) {
                             if (ks < C::PV_STEPS_PER_TILE * ntile) {
-                                // the stream's first pair (jp = 0 or 1) starts its accumulator afresh
-                                const uint32_t acc = (jp > 1) || (ks > 0);
+                                const uint32_t acc = (jp > 0) || (ks > 0);
                                 if constexpr (kFp8) mma_f8_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
                                 else mma_f16_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
                             }
                         }
                         tc_commit(bar(C::B_V_EMPTY + st));
+                        tc_commit(bar(C::B_PV_DONE + sb));
                         if (jp == it.np - 1) tc_commit(bar(C::B_ITEM_DONE));
                     }
                 }
@@ -277,14 +278,15 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     } else {
         // ======================= softmax warps ======================================================
         setmaxnreg_inc_216();
-        const int sm = warp >> 2;                // stream: pairs sm, sm + 2, ... of every item
+        const int sm = warp >> 2;                // parity: pairs sm, sm + 2, ... of every item
         const int wq = warp & 3;                 // TMEM lane quarter
         const int row = wq * 32 + lane;          // query row inside the block == TMEM lane
         const uint32_t tlane = tmem + (static_cast<uint32_t>(wq * 32) << 16);
-        const uint32_t tS = tlane + TM_S + sm * 128;          // this stream's S / P
-        const uint32_t tOs = tlane + TM_O + sm * 128;         // this stream's O accumulator
+        const uint32_t tOs = tlane + TM_O;       // the O accumulator (all 128 columns of this row)
         const int nsb = (p.N + 127) >> 7;        // FP8: Q/K scale blocks of 128 tokens
-        uint32_t cnt = 0;                        // pairs this stream has processed (phase of S_FULL)
+        volatile float* xm = xch;                // [128] m_ref hand-off between the two parities
+        volatile float* xe = xch + 128;          // [2 parity][m, l][128] epilogue exchange
+        uint32_t g0 = 0;                         // pairs of all previous items (S buffer / phase)
         uint32_t icnt = 0;                       // non-empty items so far
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
             const Item it = get_item(p, idx);
@@ -303,7 +305,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 if (2 * sm < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * sm);
                 if (2 * sm + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * sm + 1);
             }
-            for (int j = sm; j < it.np; j += 2, ++cnt) {
+            for (int j = sm; j < it.np; j += 2) {
+                const uint32_t g = g0 + j, sb = g % SBUFS;
+                const uint32_t tS = tlane + TM_S + sb * 128;     // this pair's S, overwritten by its P
                 int va = BK, vb = BK;            // valid keys in the two tiles of the pair
                 int kba = 0, kbb = 0;
                 if constexpr (kFp8) {
@@ -322,7 +326,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     va = min(BK, p.N - kba * BK);
                     vb = (2 * j + 1 < it.nt) ? min(BK, p.N - kbb * BK) : 0;
                 }
-                mbar_wait(bar(C::B_S_FULL + sm), cnt & 1);
+                mbar_wait(bar(C::B_S_FULL + sb), (g / SBUFS) & 1);
                 tc_fence_after();
                 // The 128 scores of a row are streamed from tensor memory twice, 32 columns at a time
                 // with the next chunk's load in flight (pass 1: row max; pass 2: exp, pack, store P
@@ -365,25 +369,45 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     mxb = fmaxf(mxb, max32(rb));
                 }
                 const float mt = fmaxf(mxa * sl2a, mxb * sl2b);   // sl2 > 0; va > 0
-                if (__any_sync(0xffffffffu, mt > m_ref + C::RESCALE_THRESHOLD)) {
+                // m_ref hand-off: the other parity published the reference it used for pair j - 1
+                // (and under which O now stands) after ITS max pass.
+                if (j > 0) {
+                    named_bar_sync(NB_HAND + (sm ^ 1) * 4 + wq, 64);
+                    const float m_in = xm[row];
+                    if (m_in != m_ref) {             // also covers m_ref = -inf (this warp's first pair)
+                        const float a = ex2(m_ref - m_in);
+                        l0 *= a;
+                        l1 *= a;
+                        m_ref = m_in;
+                    }
+                }
+                const bool grow = __any_sync(0xffffffffu, mt > m_ref + C::RESCALE_THRESHOLD);
+                float alpha = 1.f;
+                if (grow) {
                     const float m_new = fmaxf(m_ref, mt);
-                    const float alpha = ex2(m_ref - m_new);   // m_ref = -inf (first pair) -> 0
+                    alpha = ex2(m_ref - m_new);      // m_ref = -inf (first pair of the item) -> 0
                     l0 *= alpha;
                     l1 *= alpha;
                     m_ref = m_new;
-                    if (j >= 2) {
-                        // O_st holds this stream's earlier pairs under the old reference.  S_FULL of
-                        // pair j was committed after P V of pair j - 2 on the in-order tensor pipe,
-                        // so that product is complete and nothing else touches O_st until P_READY.
+                }
+                if (j + 1 < it.np) {                 // publish before the (rare) rescale: P V of pair j + 1
+                    xm[row] = m_ref;                 // cannot be issued before this pair's P is ready
+                    named_bar_arrive(NB_HAND + sm * 4 + wq, 64);
+                }
+                if (grow && j > 0) {
+                    // O holds pairs 0..j-1 under the old reference; wait for P V of pair j-1.
+                    // (S_FULL of pair g implies P V of pair g-3 is complete, so the barrier of
+                    // buffer (g-1) % 3 is at most one phase behind: the parity wait is exact.)
+                    mbar_wait(bar(C::B_PV_DONE + (g - 1) % SBUFS), ((g - 1) / SBUFS) & 1);
+                    tc_fence_after();
 #pragma unroll 1
-                        for (int c = 0; c < 4; ++c) {
-                            tc_wait_ld();
-                            tmem_ld32(tOs + c * 32, rb);
-                            tc_wait_ld();
+                    for (int c = 0; c < 4; ++c) {
+                        tc_wait_ld();
+                        tmem_ld32(tOs + c * 32, rb);
+                        tc_wait_ld();
 #pragma unroll
-                            for (int k = 0; k < 32; ++k) rb[k] = __float_as_uint(__uint_as_float(rb[k]) * alpha);
-                            tmem_st32(tOs + c * 32, rb);
-                        }
+                        for (int k = 0; k < 32; ++k) rb[k] = __float_as_uint(__uint_as_float(rb[k]) * alpha);
+                        tmem_st32(tOs + c * 32, rb);
                     }
                 }
                 {
@@ -447,58 +471,59 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 tc_wait_st();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(C::B_P_READY + sm));
+                if (lane == 0) mbar_arrive(bar(C::B_P_READY + sb));
             }
-            // ---------------- epilogue: merge the two streams, normalise, convert, store ----------
-            // Warp (sm, wq) finalises O columns [64 sm, 64 sm + 64) of its 32 rows from BOTH accumulators.
+            g0 += it.np;
+            // ---------------- epilogue: add the partial row sums, normalise, convert, store ------
+            // Warp (sm, wq) finalises O columns [64 sm, 64 sm + 64) of its 32 rows.  The parity that
+            // handled the last pair holds the final m_ref; the other one may be one update behind.
             const float l_mine = l0 + l1;
-            xch[(sm * 2 + 0) * 128 + row] = m_ref;
-            xch[(sm * 2 + 1) * 128 + row] = l_mine;
+            xe[(sm * 2 + 0) * 128 + row] = m_ref;
+            xe[(sm * 2 + 1) * 128 + row] = l_mine;
             if (lane == 0 && wq == 0) tma_store_wait_read();   // staging slab sm is free again
             named_bar_sync(NB_PAIR + wq, 64);
-            const float m_oth = xch[((sm ^ 1) * 2 + 0) * 128 + row];
-            const float l_oth = xch[((sm ^ 1) * 2 + 1) * 128 + row];
+            const float m_oth = xe[((sm ^ 1) * 2 + 0) * 128 + row];
+            const float l_oth = xe[((sm ^ 1) * 2 + 1) * 128 + row];
             named_bar_sync(NB_PAIR + wq, 64);                  // both have read: the slots may be rewritten
             const float m_all = fmaxf(m_ref, m_oth);
-            // a stream without pairs has m = -inf, l = 0: weight 0 and its accumulator is not read
+            // a parity without pairs has m = -inf, l = 0
             const float a_mine = (m_ref == -INFINITY) ? 0.f : ex2(m_ref - m_all);
             const float a_oth = (m_oth == -INFINITY) ? 0.f : ex2(m_oth - m_all);
             const float L = l_mine * a_mine + l_oth * a_oth;
             const float inv = (L > 0.f) ? 1.f / L : 0.f;
-            const float w0 = (sm == 0 ? a_mine : a_oth) * inv, w1 = (sm == 0 ? a_oth : a_mine) * inv;
             named_bar_sync(NB_HALF + sm, 128);                 // staging free for the whole warpgroup
             if (it.nt > 0) {
                 mbar_wait(bar(C::B_ITEM_DONE), icnt & 1);      // every P V of the item has completed
                 tc_fence_after();
             }
             const uint32_t srow = sO + sm * 16384 + row * 128;
-            const uint32_t tO0 = tlane + TM_O + sm * 64, tO1 = tlane + TM_O + 128 + sm * 64;
+            const uint32_t tO = tOs + sm * 64;
             // FP8: O[:, c] carries V's per-channel scale (R10)
             const float4* vsc = nullptr;
             if constexpr (kFp8)
                 vsc = reinterpret_cast<const float4*>(p.v_scale + (static_cast<int64_t>(it.b) * p.H + it.h) * 128 + sm * 64);
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
-                uint32_t o0[32], o1[32];
-                const bool has0 = it.nt > 0, has1 = it.np > 1;     // warp-uniform
-                if (has0) tmem_ld32(tO0 + c * 32, o0);
-                if (has1) tmem_ld32(tO1 + c * 32, o1);
-                if (has0) tc_wait_ld();
+                uint32_t o[32];
+                if (it.nt > 0) {
+                    tmem_ld32(tO + c * 32, o);
+                    tc_wait_ld();
+                }
                 uint32_t pk[16];
 #pragma unroll
                 for (int k4 = 0; k4 < 8; ++k4) {
-                    float4 sc = make_float4(1.f, 1.f, 1.f, 1.f);
-                    if constexpr (kFp8) sc = __ldg(vsc + c * 8 + k4);
-                    float x[4];
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        float v = 0.f;
-                        if (has0) v = __uint_as_float(o0[4 * k4 + e]) * w0;
-                        if (has1) v = fmaf(__uint_as_float(o1[4 * k4 + e]), w1, v);
-                        x[e] = v;
+                    float4 w = make_float4(inv, inv, inv, inv);
+                    if constexpr (kFp8) {
+                        const float4 sc = __ldg(vsc + c * 8 + k4);
+                        w = make_float4(inv * sc.x, inv * sc.y, inv * sc.z, inv * sc.w);
                     }
-                    pk[2 * k4] = pack_bf16x2(x[0] * sc.x, x[1] * sc.y);
-                    pk[2 * k4 + 1] = pack_bf16x2(x[2] * sc.z, x[3] * sc.w);
+                    float x0 = 0.f, x1 = 0.f, x2 = 0.f, x3 = 0.f;
+                    if (it.nt > 0) {
+                        x0 = __uint_as_float(o[4 * k4]) * w.x;     x1 = __uint_as_float(o[4 * k4 + 1]) * w.y;
+                        x2 = __uint_as_float(o[4 * k4 + 2]) * w.z; x3 = __uint_as_float(o[4 * k4 + 3]) * w.w;
+                    }
+                    pk[2 * k4] = pack_bf16x2(x0, x1);
+                    pk[2 * k4 + 1] = pack_bf16x2(x2, x3);
                 }
 #pragma unroll
                 for (int q4 = 0; q4 < 4; ++q4) {
