@@ -107,6 +107,16 @@ __device__ __forceinline__ Item get_item(const AttnParams& p, int idx) {
     return it;
 }
 
+// the same, with every field broadcast from lane 0: the compiler then knows the values are
+// warp-uniform (needed by the converged producer / MMA warps)
+__device__ __forceinline__ Item get_item_uniform(const AttnParams& p, int idx) {
+    Item it = get_item(p, idx);
+    it.r0 = __shfl_sync(0xffffffffu, it.r0, 0);
+    it.nt = __shfl_sync(0xffffffffu, it.nt, 0);
+    it.np = (it.nt + 1) >> 1;
+    return it;
+}
+
 __device__ __forceinline__ float max3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
 
 // max of 64 fp32 bit patterns
@@ -171,7 +181,12 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp >= 8) {
         // ======================= producer / MMA warpgroup ==========================================
         setmaxnreg_dec_56();
-        if (warp == PRODUCER_WARP && lane == 0) {
+        // Both roles run with the WHOLE warp converged (all lanes wait on the barriers and keep the
+        // same loop state); one elected lane issues the TMA / tcgen05 instructions.  Everything an
+        // issue needs is made warp-uniform with a shuffle first, so that the compiler keeps the
+        // descriptors and coordinates in uniform registers instead of wrapping every issue in a
+        // per-lane loop (which made the single-thread issue stream the bottleneck of the kernel).
+        if (warp == PRODUCER_WARP) {
             // one 128-row, 128-channel box = SLABS loads of [rows][128 B]
             auto load_tile = [&](uint32_t dst, const CUtensorMap* tm, uint32_t b, int row0, int h, int bb) {
                 tma_load_4d(dst, tm, b, 0, row0, h, bb);
@@ -179,35 +194,50 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             };
             uint32_t g = 0, icnt = 0;   // pairs and non-empty items issued so far
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
-                const Item it = get_item(p, idx);
+                const Item it = get_item_uniform(p, idx);
                 if (it.nt == 0) continue;   // empty rows touch no barrier
                 mbar_wait(bar(C::B_Q_EMPTY), (icnt & 1) ^ 1);
-                mbar_arrive_expect_tx(bar(C::B_Q_FULL), TILE);
-                load_tile(sQ, &tmQ, bar(C::B_Q_FULL), it.qb * BQ, it.h, it.b);
-                for (int j = 0; j < it.np; ++j, ++g) {
-                    const int ntile = (2 * j + 1 < it.nt) ? 2 : 1;
-                    const int kb0 = __ldg(p.col_idx + it.r0 + 2 * j);
-                    const int kb1 = (ntile == 2) ? __ldg(p.col_idx + it.r0 + 2 * j + 1) : 0;
-                    {
-                        const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1;
-                        mbar_wait(bar(C::B_K_EMPTY + st), ph ^ 1);
-                        mbar_arrive_expect_tx(bar(C::B_K_FULL + st), ntile * (TILE / 2));
-                        const uint32_t dst = sK + st * TILE;
-                        load_tile(dst, &tmK, bar(C::B_K_FULL + st), kb0 * BK, it.h, it.b);
-                        if (ntile == 2) load_tile(dst + HALF, &tmK, bar(C::B_K_FULL + st), kb1 * BK, it.h, it.b);
-                    }
-                    {
-                        const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1;
-                        mbar_wait(bar(C::B_V_EMPTY + st), ph ^ 1);
-                        mbar_arrive_expect_tx(bar(C::B_V_FULL + st), ntile * (TILE / 2));
-                        const uint32_t dst = sV + st * TILE;
-                        load_tile(dst, &tmV, bar(C::B_V_FULL + st), kb0 * BK, it.h, it.b);
-                        if (ntile == 2) load_tile(dst + HALF, &tmV, bar(C::B_V_FULL + st), kb1 * BK, it.h, it.b);
+                if (elect_one()) {
+                    mbar_arrive_expect_tx(bar(C::B_Q_FULL), TILE);
+                    load_tile(sQ, &tmQ, bar(C::B_Q_FULL), it.qb * BQ, it.h, it.b);
+                }
+                __syncwarp();
+                // the key-block indices of 16 pairs are fetched with one coalesced load
+                for (int j0 = 0; j0 < it.np; j0 += 16) {
+                    const int t = 2 * j0 + lane;
+                    const int mine = (t < it.nt) ? __ldg(p.col_idx + it.r0 + t) : 0;
+                    const int jn = min(16, it.np - j0);
+                    for (int jl = 0; jl < jn; ++jl, ++g) {
+                        const int ntile = (2 * (j0 + jl) + 1 < it.nt) ? 2 : 1;
+                        const int kb0 = __shfl_sync(0xffffffffu, mine, 2 * jl);
+                        const int kb1 = __shfl_sync(0xffffffffu, mine, 2 * jl + 1);
+                        {
+                            const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1;
+                            mbar_wait(bar(C::B_K_EMPTY + st), ph ^ 1);
+                            if (elect_one()) {
+                                mbar_arrive_expect_tx(bar(C::B_K_FULL + st), ntile * (TILE / 2));
+                                const uint32_t dst = sK + st * TILE;
+                                load_tile(dst, &tmK, bar(C::B_K_FULL + st), kb0 * BK, it.h, it.b);
+                                if (ntile == 2) load_tile(dst + HALF, &tmK, bar(C::B_K_FULL + st), kb1 * BK, it.h, it.b);
+                            }
+                            __syncwarp();
+                        }
+                        {
+                            const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1;
+                            mbar_wait(bar(C::B_V_EMPTY + st), ph ^ 1);
+                            if (elect_one()) {
+                                mbar_arrive_expect_tx(bar(C::B_V_FULL + st), ntile * (TILE / 2));
+                                const uint32_t dst = sV + st * TILE;
+                                load_tile(dst, &tmV, bar(C::B_V_FULL + st), kb0 * BK, it.h, it.b);
+                                if (ntile == 2) load_tile(dst + HALF, &tmV, bar(C::B_V_FULL + st), kb1 * BK, it.h, it.b);
+                            }
+                            __syncwarp();
+                        }
                     }
                 }
                 ++icnt;
             }
-        } else if (warp == MMA_WARP && lane == 0) {
+        } else if (warp == MMA_WARP) {
             // kind::f16: format 1 = bf16; kind::f8f6f4: format 0 = e4m3.  PV: B (= V) is MN-major.
             constexpr uint32_t FMT = kFp8 ? 0u : 1u;
             constexpr uint32_t IDESC_S128 = make_idesc(FMT, FMT, 128, 128, 0, 0);
@@ -218,57 +248,69 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const uint64_t dV = smem_desc_sw128(sV, 16384, 1024);
             uint32_t g0 = 0, icnt = 0;      // pairs before this item, non-empty items so far
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
-                const Item it = get_item(p, idx);
+                const Item it = get_item_uniform(p, idx);
                 if (it.nt == 0) continue;
                 mbar_wait(bar(C::B_Q_FULL), icnt & 1);
                 for (int jj = 0; jj < it.np + 2; ++jj) {
                     if (jj < it.np) {   // S[g % 3] = Q K^T of pair jj (runs up to two pairs ahead)
                         const uint32_t g = g0 + jj;
                         const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1, sb = g % SBUFS;
-                        const int ntile = (2 * jj + 1 < it.nt) ? 2 : 1;
+                        const bool two = 2 * jj + 1 < it.nt;
                         mbar_wait(bar(C::B_K_FULL + st), ph);
                         tc_fence_after();
-                        const uint32_t tS = tmem + TM_S + sb * 128;
-                        const uint32_t idesc = (ntile == 2) ? IDESC_S128 : IDESC_S64;
-                        const uint64_t dKs = dK + ((st * TILE) >> 4);
-                        if constexpr (kFp8) {
+                        if (elect_one()) {
+                            const uint32_t tS = tmem + TM_S + sb * 128;
+                            const uint32_t idesc = two ? IDESC_S128 : IDESC_S64;
+                            const uint64_t dKs = dK + ((st * TILE) >> 4);
+                            if constexpr (kFp8) {
 #pragma unroll
-                            for (int ks = 0; ks < 4; ++ks)       // 32 e4m3 channels = 32 B per step
-                                mma_f8_ss(tS, dQ + ((ks * 32) >> 4), dKs + ((ks * 32) >> 4), idesc, ks > 0);
-                        } else {
+                                for (int ks = 0; ks < 4; ++ks)       // 32 e4m3 channels = 32 B per step
+                                    mma_f8_ss(tS, dQ + ((ks * 32) >> 4), dKs + ((ks * 32) >> 4), idesc, ks > 0);
+                            } else {
 #pragma unroll
-                            for (int ks = 0; ks < 8; ++ks) {     // 16 bf16 channels = 32 B per step, 2 slabs
-                                const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
-                                mma_f16_ss(tS, dQ + off, dKs + off, idesc, ks > 0);
+                                for (int ks = 0; ks < 8; ++ks) {     // 16 bf16 channels = 32 B per step, 2 slabs
+                                    const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
+                                    mma_f16_ss(tS, dQ + off, dKs + off, idesc, ks > 0);
+                                }
                             }
+                            tc_commit(bar(C::B_K_EMPTY + st));
+                            tc_commit(bar(C::B_S_FULL + sb));
+                            if (jj == it.np - 1) tc_commit(bar(C::B_Q_EMPTY));
                         }
-                        tc_commit(bar(C::B_K_EMPTY + st));
-                        tc_commit(bar(C::B_S_FULL + sb));
-                        if (jj == it.np - 1) tc_commit(bar(C::B_Q_EMPTY));
+                        __syncwarp();
                     }
                     if (jj >= 2) {      // O += P V of pair jj - 2
                         const int jp = jj - 2;
                         const uint32_t g = g0 + jp;
                         const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1, sb = g % SBUFS;
-                        const int ntile = (2 * jp + 1 < it.nt) ? 2 : 1;
+                        const bool two = 2 * jp + 1 < it.nt;
                         mbar_wait(bar(C::B_P_READY + sb), (g / SBUFS) & 1);
                         mbar_wait(bar(C::B_V_FULL + st), ph);
                         if (jp == 0) mbar_wait(bar(C::B_O_FREE), (icnt & 1) ^ 1);
                         tc_fence_after();
-                        const uint32_t tP = tmem + TM_S + sb * 128, tO = tmem + TM_O;
-                        const uint64_t dVs = dV + ((st * TILE) >> 4);
-                        constexpr uint32_t KBYTES = kFp8 ? 4096u : 2048u;   // 32 / 16 keys x 128 B per step
+                        if (elect_one()) {
+                            const uint32_t tP = tmem + TM_S + sb * 128, tO = tmem + TM_O;
+                            const uint64_t dVs = dV + ((st * TILE) >> 4);
+                            constexpr uint32_t KBYTES = kFp8 ? 4096u : 2048u;   // 32 / 16 keys x 128 B per step
+                            constexpr int STEPS = C::PV_STEPS_PER_TILE;
 #pragma unroll
-                        for (int ks = 0; ks < 2 * C::PV_STEPS_PER_TILE; ++ks) {
-                            if (ks < C::PV_STEPS_PER_TILE * ntile) {
+                            for (int ks = 0; ks < STEPS; ++ks) {
                                 const uint32_t acc = (jp > 0) || (ks > 0);
                                 if constexpr (kFp8) mma_f8_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
                                 else mma_f16_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
                             }
+                            if (two) {
+#pragma unroll
+                                for (int ks = STEPS; ks < 2 * STEPS; ++ks) {
+                                    if constexpr (kFp8) mma_f8_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, 1u);
+                                    else mma_f16_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, 1u);
+                                }
+                            }
+                            tc_commit(bar(C::B_V_EMPTY + st));
+                            tc_commit(bar(C::B_PV_DONE + sb));
+                            if (jp == it.np - 1) tc_commit(bar(C::B_ITEM_DONE));
                         }
-                        tc_commit(bar(C::B_V_EMPTY + st));
-                        tc_commit(bar(C::B_PV_DONE + sb));
-                        if (jp == it.np - 1) tc_commit(bar(C::B_ITEM_DONE));
+                        __syncwarp();
                     }
                 }
                 g0 += it.np;
