@@ -29,6 +29,8 @@
 // 64-key tile and V's per-channel scale applied in the epilogue.
 #include <cuda_bf16.h>
 
+#include <cstdio>
+
 #include "chorus_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -37,6 +39,18 @@ namespace {
 
 using namespace ptx;
 
+#ifndef CHORUS_EXP_TOKEN
+#define CHORUS_EXP_TOKEN 0
+#endif
+// debug only: per-phase cycle counters of the softmax warps of CTA 0, printed at kernel exit
+#ifndef CHORUS_PHASE_CLOCKS
+#define CHORUS_PHASE_CLOCKS 0
+#endif
+#if CHORUS_PHASE_CLOCKS
+#define PHASE_MARK(i) do { const long long t_ = clock64(); ph_acc[i] += t_ - ph_t; ph_t = t_; } while (0)
+#else
+#define PHASE_MARK(i) do { } while (0)
+#endif
 #ifndef CHORUS_POLY_MASK
 #define CHORUS_POLY_MASK 0x00u   // e.g. 0x4A = 3 of every 8 element pairs
 #endif
@@ -90,6 +104,11 @@ constexpr uint32_t NB_PAIR = 1, NB_HALF = 5, NB_HAND = 7;
 
 __device__ __forceinline__ void setmaxnreg_inc_216() { asm volatile("setmaxnreg.inc.sync.aligned.u32 216;"); }
 __device__ __forceinline__ void setmaxnreg_dec_56() { asm volatile("setmaxnreg.dec.sync.aligned.u32 56;"); }
+
+template <bool V>
+struct BoolTag {
+    static constexpr bool value = V;
+};
 
 struct Item {
     int b, h, qb, r0, nt, np;
@@ -330,6 +349,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         volatile float* xe = xch + 128;          // [2 parity][m, l][128] epilogue exchange
         uint32_t g0 = 0;                         // pairs of all previous items (S buffer / phase)
         uint32_t icnt = 0;                       // non-empty items so far
+#if CHORUS_PHASE_CLOCKS
+        long long ph_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, ph_t = clock64();
+        const long long ph_t0 = ph_t;
+        int ph_pairs = 0;
+#endif
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
             const Item it = get_item(p, idx);
             float m_ref = -INFINITY, l0 = 0.f, l1 = 0.f;
@@ -368,12 +392,18 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     va = min(BK, p.N - kba * BK);
                     vb = (2 * j + 1 < it.nt) ? min(BK, p.N - kbb * BK) : 0;
                 }
+                PHASE_MARK(0);
                 mbar_wait(bar(C::B_S_FULL + sb), (g / SBUFS) & 1);
                 tc_fence_after();
+                PHASE_MARK(1);
                 // The 128 scores of a row are streamed from tensor memory twice, 32 columns at a time
                 // with the next chunk's load in flight (pass 1: row max; pass 2: exp, pack, store P
                 // behind the read position), so that only 64 of them are ever live in registers.
                 const bool ragged = (va < BK) || (vb < BK);   // warp-uniform, last pair of a row only
+                // The body is instantiated twice (with / without tail masking) so that the common
+                // case carries no branch: the compiler can then schedule across the chunks.
+                auto pair_body = [&](auto rag_tag) {
+                constexpr bool RAG = decltype(rag_tag)::value;
                 auto mask_chunk = [&](uint32_t (&r)[32], int c) {
                     const int valid = ((c >> 1) ? vb : va) - 32 * (c & 1);
 #pragma unroll
@@ -395,22 +425,23 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     tmem_ld32(tS, ra);
                     tc_wait_ld();
                     tmem_ld32(tS + 32, rb);
-                    if (ragged) mask_chunk(ra, 0);
+                    if constexpr (RAG) mask_chunk(ra, 0);
                     mxa = max32(ra);
                     tc_wait_ld();
                     tmem_ld32(tS + 64, ra);
-                    if (ragged) mask_chunk(rb, 1);
+                    if constexpr (RAG) mask_chunk(rb, 1);
                     mxa = fmaxf(mxa, max32(rb));
                     tc_wait_ld();
                     tmem_ld32(tS + 96, rb);
-                    if (ragged) mask_chunk(ra, 2);
+                    if constexpr (RAG) mask_chunk(ra, 2);
                     mxb = max32(ra);
                     tc_wait_ld();
                     tmem_ld32(tS, ra);                       // first chunk of pass 2
-                    if (ragged) mask_chunk(rb, 3);
+                    if constexpr (RAG) mask_chunk(rb, 3);
                     mxb = fmaxf(mxb, max32(rb));
                 }
                 const float mt = fmaxf(mxa * sl2a, mxb * sl2b);   // sl2 > 0; va > 0
+                PHASE_MARK(2);
                 // m_ref hand-off: the other parity published the reference it used for pair j - 1
                 // (and under which O now stands) after ITS max pass.
                 if (j > 0) {
@@ -434,8 +465,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 }
                 if (j + 1 < it.np) {                 // publish before the (rare) rescale: P V of pair j + 1
                     xm[row] = m_ref;                 // cannot be issued before this pair's P is ready
+#if !CHORUS_EXP_TOKEN
                     named_bar_arrive(NB_HAND + sm * 4 + wq, 64);
+#endif
                 }
+                PHASE_MARK(3);
                 if (grow && j > 0) {
                     // O holds pairs 0..j-1 under the old reference; wait for P V of pair j-1.
                     // (S_FULL of pair g implies P V of pair g-3 is complete, so the barrier of
@@ -494,27 +528,42 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     };
                     tc_wait_ld();
                     tmem_ld32(tS + 32, rb);
-                    if (ragged) mask_chunk(ra, 0);
+                    if constexpr (RAG) mask_chunk(ra, 0);
                     exp_chunk(ra, 0);
                     tc_wait_ld();
                     tmem_ld32(tS + 64, ra);
-                    if (ragged) mask_chunk(rb, 1);
+                    if constexpr (RAG) mask_chunk(rb, 1);
                     exp_chunk(rb, 1);
                     tc_wait_ld();
                     tmem_ld32(tS + 96, rb);
-                    if (ragged) mask_chunk(ra, 2);
+                    if constexpr (RAG) mask_chunk(ra, 2);
                     exp_chunk(ra, 2);
                     tc_wait_ld();
-                    if (ragged) mask_chunk(rb, 3);
+                    if constexpr (RAG) mask_chunk(rb, 3);
                     exp_chunk(rb, 3);
                     l0 = lacc.x;
                     l1 = lacc.y;
                 }
+#if CHORUS_EXP_TOKEN
+                // The hand-off doubles as an exp-phase token: the other parity starts its exp pass
+                // only now, so the two warps of a sub-partition never compete for the MUFU and one
+                // of them is always in its (MUFU-free) load / max phase.
+                if (j + 1 < it.np) named_bar_arrive(NB_HAND + sm * 4 + wq, 64);
+#endif
+                };
+                if (ragged) pair_body(BoolTag<true>{});
+                else pair_body(BoolTag<false>{});
+                PHASE_MARK(4);
                 tc_wait_st();
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(C::B_P_READY + sb));
+                PHASE_MARK(5);
+#if CHORUS_PHASE_CLOCKS
+                ++ph_pairs;
+#endif
             }
+            PHASE_MARK(0);
             g0 += it.np;
             // ---------------- epilogue: add the partial row sums, normalise, convert, store ------
             // Warp (sm, wq) finalises O columns [64 sm, 64 sm + 64) of its 32 rows.  The parity that
@@ -589,6 +638,14 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             }
         }
         if (lane == 0 && wq == 0) tma_store_wait_all();
+#if CHORUS_PHASE_CLOCKS
+        PHASE_MARK(6);
+        if (blockIdx.x == 0 && lane == 0 && wq == 1)
+            printf("phase clocks warp %d: pairs %d total %lld | per pair: top %lld waitS %lld max %lld hand %lld exp %lld "
+                   "st+arrive %lld | epilogue total %lld\n", warp, ph_pairs, clock64() - ph_t0, ph_acc[0] / ph_pairs,
+                   ph_acc[1] / ph_pairs, ph_acc[2] / ph_pairs, ph_acc[3] / ph_pairs, ph_acc[4] / ph_pairs,
+                   ph_acc[5] / ph_pairs, ph_acc[6]);
+#endif
     }
     tc_fence_before();
     __syncthreads();
