@@ -105,7 +105,7 @@ chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq
     if (rows * nk_blk > INT32_MAX)
         return set_error(CHORUS_ERR_CAPACITY, "L*H*nq_blk*nk_blk = %lld exceeds INT32_MAX",
                          static_cast<long long>(rows * nk_blk));
-    const size_t need = decode_workspace_bytes(rows);
+    const size_t need = decode_workspace_bytes(rows, (nk_blk + 31) / 32);
     if (!workspace) {
         *workspace_bytes = need;
         return CHORUS_OK;

@@ -14,7 +14,7 @@ chorus_status check_cuda(cudaError_t e, const char* what);
 void count_launch(int n = 1);
 
 // ---- mask_decode.cu ----------------------------------------------------------------------------
-size_t decode_workspace_bytes(int64_t rows);
+size_t decode_workspace_bytes(int64_t rows, int words);
 cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, int words,
                                int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
                                cudaStream_t stream);

@@ -1,16 +1,17 @@
 // mask_decode.cu — chorus_mask_to_index and chorus_visit_refresh kernels (HBM-bound integer work).
 //
 // Decode (PAPER.md:L81/L87/L93; include/chorus.h): packed block bitmask [rows][words] ->
-// CSR (row_ptr, col_idx), ascending inside each row.  Three launches:
-//   1. count_rows:   one warp per row: popcount of the valid bits -> row_ptr[r+1] holds the row's
-//                    count; each block also writes the sum of its ROWS_PER_BLOCK rows.
-//   2. scan_blocks:  one block turns the per-block sums into exclusive offsets.
-//   3. scatter_rows: each block scans its rows' counts (block offset + local exclusive scan),
-//                    writes the final row_ptr, and each warp expands its rows' set bits through a
-//                    shared-memory staging buffer so that col_idx is written in contiguous,
-//                    coalesced runs.
-// Algorithmic traffic: 4*(rows*words) read + 4*(rows+1) + 4*nnz written (the bitmask is read a
-// second time by launch 3; for every workload here it is still L2-resident).
+// CSR (row_ptr, col_idx), ascending inside each row.  ONE pass over the bitmask, one launch (plus a
+// memset of the small look-back array): the bitmask is taken as a flat array of rows*words words,
+// cut into tiles of 1024 words (four sub-tiles of 256, one word per thread each); a block
+//   1. loads its tile (coalesced), clears the pad bits of the last word of each row and counts;
+//   2. scans the counts inside the block and gets the number of set bits in front of its tile with
+//      a decoupled look-back over the per-tile status words, 256 at a time (tiles are taken in
+//      ticket order, so a tile only ever waits for tiles that already run);
+//   3. writes row_ptr for every row that begins in the tile, then, sub-tile by sub-tile, every
+//      thread walks the set bits of its word into a shared-memory staging buffer, which the block
+//      copies to col_idx in contiguous, coalesced runs.
+// Algorithmic traffic: 4*(rows*words) read + 4*(rows+1) + 4*nnz written; nothing is read twice.
 #include <algorithm>
 
 #include "chorus_internal.h"
@@ -20,151 +21,145 @@ namespace {
 
 constexpr int DEC_THREADS = 256;
 constexpr int DEC_WARPS = DEC_THREADS / 32;
-constexpr int ROWS_PER_WARP = 16;
-constexpr int ROWS_PER_BLOCK = DEC_WARPS * ROWS_PER_WARP;  // 128
+constexpr int SUBTILES = 4;
+constexpr int TILE_WORDS = DEC_THREADS * SUBTILES;   // 1024 words = up to 32768 key blocks
+constexpr int STAGE = DEC_THREADS * 32;              // one sub-tile can never hold more entries
 
-__device__ __forceinline__ uint32_t valid_word(const uint32_t* __restrict__ row, int w, int nk) {
-    // word w of a row with the pad bits (>= nk) cleared; 0 beyond the row
-    const int lo = w * 32;
-    if (lo >= nk) return 0u;
-    uint32_t v = __ldg(row + w);
-    const int rem = nk - lo;
-    if (rem < 32) v &= (1u << rem) - 1u;
+// per-tile status word: bits 63..62 = state (0 empty, 1 aggregate of the tile, 2 inclusive prefix),
+// low 32 bits = value.  Written and read with single 64-bit relaxed accesses.
+constexpr unsigned long long ST_AGG = 1ull << 62, ST_INC = 2ull << 62;
+
+__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
 
 __global__ void __launch_bounds__(DEC_THREADS)
-count_rows_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, int words,
-                  int32_t* __restrict__ row_ptr, int32_t* __restrict__ block_sums) {
-    __shared__ int warp_sums[DEC_WARPS];
+decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, int words,
+                    int32_t* __restrict__ row_ptr, int32_t* __restrict__ col_idx, int64_t col_cap,
+                    unsigned long long* __restrict__ status /* [0] = ticket counter, [1 + t] = tile t */) {
+    // entry e sits at e + e/32: threads whose runs start 8, 16 or 32 entries apart (25 %, 50 %, full
+    // density) then hit different banks when they all write their k-th entry
+    __shared__ int32_t s_stage[STAGE + STAGE / 32];
+    __shared__ int s_warp[SUBTILES][DEC_WARPS];
+    __shared__ int2 s_look[DEC_WARPS];
+    __shared__ int s_tile, s_base;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t row0 = static_cast<int64_t>(blockIdx.x) * ROWS_PER_BLOCK + warp * ROWS_PER_WARP;
-    int wsum = 0;
-    for (int i = 0; i < ROWS_PER_WARP; ++i) {
-        const int64_t r = row0 + i;
-        if (r >= rows) break;
-        const uint32_t* row = bitmask + r * words;
-        int c = 0;
-        for (int w = lane; w < words; w += 32) c += __popc(valid_word(row, w, nk));
-        c = __reduce_add_sync(0xffffffffu, c);
-        if (lane == 0) row_ptr[r + 1] = c;
-        wsum += c;
-    }
-    if (lane == 0) warp_sums[warp] = wsum;
+    if (threadIdx.x == 0) s_tile = static_cast<int>(atomicAdd(status, 1ull));
     __syncthreads();
-    if (threadIdx.x == 0) {
-        int s = 0;
-        for (int w = 0; w < DEC_WARPS; ++w) s += warp_sums[w];
-        block_sums[blockIdx.x] = s;
-    }
-}
+    const int tile = s_tile;
+    // all word indices fit 32 bits: rows * nk <= INT32_MAX is checked by the caller
+    const uint32_t n_words = static_cast<uint32_t>(rows * words);
+    const uint32_t tile0 = static_cast<uint32_t>(tile) * TILE_WORDS;
+    const int rem = nk - (words - 1) * 32;                      // valid bits of a row's last word
+    const uint32_t last_mask = rem >= 32 ? 0xffffffffu : ((1u << rem) - 1u);
 
-// exclusive scan of block_sums (n entries) in place; one block of 1024 threads
-__global__ void __launch_bounds__(1024)
-scan_blocks_kernel(int32_t* __restrict__ block_sums, int n) {
-    __shared__ int warp_tot[32];
-    __shared__ int carry_s;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (int base = 0; base < n; base += 1024) {
-        const int i = base + threadIdx.x;
-        const int v = (i < n) ? block_sums[i] : 0;
-        int inc = v;
+    // 1. load (word tile0 + 256 s + thread for sub-tile s), mask the pad bits, count
+    uint32_t v[SUBTILES];
+    int win[SUBTILES], rowi[SUBTILES], cnt[SUBTILES], inc[SUBTILES];
+#pragma unroll
+    for (int sidx = 0; sidx < SUBTILES; ++sidx) {
+        const uint32_t w = tile0 + sidx * DEC_THREADS + threadIdx.x;
+        const uint32_t r = w / static_cast<uint32_t>(words);
+        const int wr = static_cast<int>(w - r * static_cast<uint32_t>(words));
+        uint32_t x = (w < n_words) ? __ldg(bitmask + w) : 0u;
+        if (wr == words - 1) x &= last_mask;
+        v[sidx] = x;
+        win[sidx] = wr;
+        rowi[sidx] = static_cast<int>(r);
+        cnt[sidx] = __popc(x);
+        // 2a. inclusive scan inside the warp
+        int t = cnt[sidx];
+#pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
+            const int u = __shfl_up_sync(0xffffffffu, t, o);
+            if (lane >= o) t += u;
         }
-        if (lane == 31) warp_tot[warp] = inc;
-        __syncthreads();
-        if (warp == 0) {
-            int t = warp_tot[lane];
-            int ti = t;
-            for (int o = 1; o < 32; o <<= 1) {
-                const int u = __shfl_up_sync(0xffffffffu, ti, o);
-                if (lane >= o) ti += u;
+        inc[sidx] = t;
+        if (lane == 31) s_warp[sidx][warp] = t;
+    }
+    __syncthreads();
+    // 2b. offsets of this thread's four words inside the tile, and the tile total
+    int off[SUBTILES], sub_total[SUBTILES], tile_total = 0;
+#pragma unroll
+    for (int sidx = 0; sidx < SUBTILES; ++sidx) {
+        int before = 0, tot = 0;
+#pragma unroll
+        for (int w = 0; w < DEC_WARPS; ++w) {
+            const int u = s_warp[sidx][w];
+            if (w < warp) before += u;
+            tot += u;
+        }
+        off[sidx] = tile_total + before + inc[sidx] - cnt[sidx];
+        sub_total[sidx] = tot;
+        tile_total += tot;
+    }
+    // 2c. decoupled look-back, 256 predecessor tiles per step (thread i looks at tile look - i): with
+    // a thousand tiles in flight the nearest tile that already knows its prefix is that far back
+    {
+        unsigned long long* mine = status + 1 + tile;
+        if (threadIdx.x == 0)
+            st_status(mine, (tile == 0 ? ST_INC : ST_AGG) | static_cast<uint32_t>(tile_total));
+        int base = 0;
+        for (int look = tile - 1; tile > 0;) {
+            const int t = look - static_cast<int>(threadIdx.x);
+            unsigned long long sv = ST_INC;         // in front of tile 0: prefix 0
+            if (t >= 0) {
+                do { sv = ld_status(status + 1 + t); } while ((sv >> 62) == 0);
             }
-            warp_tot[lane] = ti - t;  // exclusive prefix of the warp totals
+            const unsigned inc_mask = __ballot_sync(0xffffffffu, (sv >> 62) == 2);
+            const int first_inc = __ffs(inc_mask) - 1;              // nearest one in this warp's window
+            const int val = (inc_mask == 0 || lane <= first_inc) ? static_cast<int>(sv & 0xffffffffu) : 0;
+            const int wsum = __reduce_add_sync(0xffffffffu, val);
+            __syncthreads();                        // s_look is free (previous step / s_warp users done)
+            if (lane == 0) s_look[warp] = make_int2(wsum, inc_mask != 0);
+            __syncthreads();
+            bool done = false;
+#pragma unroll
+            for (int w = 0; w < DEC_WARPS; ++w) {   // warp 0 holds the nearest predecessors
+                const int2 u = s_look[w];
+                if (!done) base += u.x;
+                done = done || (u.y != 0);
+            }
+            if (done) break;
+            look -= DEC_THREADS;
         }
-        __syncthreads();
-        const int carry = carry_s;
-        if (i < n) block_sums[i] = carry + warp_tot[warp] + inc - v;
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = carry + warp_tot[warp] + inc;
-        __syncthreads();
-    }
-}
-
-__global__ void __launch_bounds__(DEC_THREADS)
-scatter_rows_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, int words,
-                    int32_t* __restrict__ row_ptr, const int32_t* __restrict__ block_offsets,
-                    int32_t* __restrict__ col_idx, int64_t col_cap) {
-    __shared__ int s_cnt[ROWS_PER_BLOCK];
-    __shared__ int s_off[ROWS_PER_BLOCK + 1];
-    __shared__ int32_t s_stage[DEC_WARPS][1024];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t blk_row0 = static_cast<int64_t>(blockIdx.x) * ROWS_PER_BLOCK;
-
-    // counts of this block's rows (written by launch 1 into row_ptr[r+1])
-    if (threadIdx.x < ROWS_PER_BLOCK) {
-        const int64_t r = blk_row0 + threadIdx.x;
-        s_cnt[threadIdx.x] = (r < rows) ? row_ptr[r + 1] : 0;
+        if (tile > 0 && threadIdx.x == 0) st_status(mine, ST_INC | static_cast<uint32_t>(base + tile_total));
+        if (threadIdx.x == 0) s_base = base;
     }
     __syncthreads();
-    // exclusive scan of 128 counts by warp 0 (4 per lane)
-    if (warp == 0) {
-        int v[4], tot = 0;
+    const int64_t base = s_base;
+    // 3a. row_ptr of the rows that begin in this tile; the thread holding the last word writes the total
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { v[k] = s_cnt[lane * 4 + k]; tot += v[k]; }
-        int inc = tot;
-        for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
-        }
-        int run = block_offsets[blockIdx.x] + inc - tot;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { s_off[lane * 4 + k] = run; run += v[k]; }
-        if (lane == 31) s_off[ROWS_PER_BLOCK] = run;
+    for (int sidx = 0; sidx < SUBTILES; ++sidx) {
+        const uint32_t w = tile0 + sidx * DEC_THREADS + threadIdx.x;
+        if (win[sidx] == 0 && w < n_words) row_ptr[rowi[sidx]] = static_cast<int32_t>(base + off[sidx]);
+        if (w == n_words - 1) row_ptr[rows] = static_cast<int32_t>(base + tile_total);
     }
-    __syncthreads();
-    // final row_ptr: row_ptr[r+1] = offset of row r+1 = off[r] + cnt[r]
-    if (threadIdx.x < ROWS_PER_BLOCK) {
-        const int64_t r = blk_row0 + threadIdx.x;
-        if (r < rows) row_ptr[r + 1] = s_off[threadIdx.x + 1];
-    }
-    if (blockIdx.x == 0 && threadIdx.x == 0) row_ptr[0] = 0;
     if (col_idx == nullptr) return;
-
-    int32_t* stage = s_stage[warp];
-    for (int i = 0; i < ROWS_PER_WARP; ++i) {
-        const int lr = warp * ROWS_PER_WARP + i;
-        const int64_t r = blk_row0 + lr;
-        if (r >= rows) break;
-        const uint32_t* row = bitmask + r * words;
-        int64_t out = s_off[lr];
-        // 32 words (1024 key blocks) per pass
-        for (int w0 = 0; w0 < words; w0 += 32) {
-            uint32_t v = valid_word(row, w0 + lane, (w0 + lane < words) ? nk : 0);
-            const int c = __popc(v);
-            int inc = c;
-            for (int o = 1; o < 32; o <<= 1) {
-                const int t = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += t;
-            }
-            const int total = __shfl_sync(0xffffffffu, inc, 31);
-            int e = inc - c;
-            const int kb0 = (w0 + lane) * 32;
-            while (v) {
-                const int b = __ffs(v) - 1;
-                stage[e++] = kb0 + b;
-                v &= v - 1;
-            }
-            __syncwarp();
-            for (int t = lane; t < total; t += 32)
-                if (out + t < col_cap) col_idx[out + t] = stage[t];
-            __syncwarp();
-            out += total;
+    // 3b. expand sub-tile by sub-tile through the staging buffer
+    int sub0 = 0;
+#pragma unroll
+    for (int sidx = 0; sidx < SUBTILES; ++sidx) {
+        uint32_t x = v[sidx];
+        const int kb0 = win[sidx] * 32;
+        int e = off[sidx] - sub0;
+        while (x) {
+            const int b = __ffs(x) - 1;
+            x &= x - 1;
+            s_stage[e + (e >> 5)] = kb0 + b;
+            ++e;
         }
+        __syncthreads();
+        const int64_t dst0 = base + sub0;
+        for (int t = threadIdx.x; t < sub_total[sidx]; t += DEC_THREADS)
+            if (dst0 + t < col_cap) col_idx[dst0 + t] = s_stage[t + (t >> 5)];
+        __syncthreads();
+        sub0 += sub_total[sidx];
     }
 }
 
@@ -186,24 +181,25 @@ visit_refresh_kernel(uint32_t* __restrict__ bitmask, int n_groups, int64_t words
     }
 }
 
-inline int64_t n_blocks_for(int64_t rows) { return (rows + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK; }
+inline int64_t n_tiles_for(int64_t rows, int words) { return (rows * words + TILE_WORDS - 1) / TILE_WORDS; }
 
 }  // namespace
 
-size_t decode_workspace_bytes(int64_t rows) {
-    return static_cast<size_t>(n_blocks_for(rows)) * sizeof(int32_t);
+size_t decode_workspace_bytes(int64_t rows, int words) {
+    // ticket counter + one status word per tile, + 8 so that the array can be 8-byte aligned
+    return static_cast<size_t>(n_tiles_for(rows, words) + 1) * sizeof(unsigned long long) + 8;
 }
 
 cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, int words,
                                int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
                                cudaStream_t stream) {
-    const int nb = static_cast<int>(n_blocks_for(rows));
-    int32_t* block_sums = static_cast<int32_t*>(workspace);
-    count_rows_kernel<<<nb, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, block_sums);
-    scan_blocks_kernel<<<1, 1024, 0, stream>>>(block_sums, nb);
-    scatter_rows_kernel<<<nb, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr,
-                                                        block_sums, col_idx, col_cap);
-    count_launch(3);
+    const int64_t nt = n_tiles_for(rows, words);
+    auto* status = reinterpret_cast<unsigned long long*>((reinterpret_cast<uintptr_t>(workspace) + 7) & ~uintptr_t(7));
+    cudaError_t e = cudaMemsetAsync(status, 0, static_cast<size_t>(nt + 1) * sizeof(unsigned long long), stream);
+    if (e != cudaSuccess) return e;
+    decode_tiles_kernel<<<static_cast<unsigned>(nt), DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr,
+                                                                             col_idx, col_cap, status);
+    count_launch(1);
     return cudaGetLastError();
 }
 
