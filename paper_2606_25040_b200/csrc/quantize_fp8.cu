@@ -26,6 +26,21 @@ __device__ __forceinline__ uint32_t cvt4_e4m3(float a, float b, float c, float d
 __device__ __forceinline__ float scale_from_amax(float amax) {
     return __fdiv_rn(fmaxf(amax, 1e-12f), 448.0f);
 }
+// RN(x / s) for many x and one s: r = RN(1 / s) is computed once; per element a product and two
+// FMA corrections (the second is exact-rounding by Markstein's theorem once the first has brought
+// the quotient within an ulp).  |x / s| <= 448 and s >= 2.2e-15, so nothing over- or underflows on
+// the way (quotients below 2^-10 round to the code 0 whatever their last bit is).  The generic
+// __fdiv_rn costs about three times as many instructions, which made the cast compute-bound.
+struct Divisor {
+    float s, r;
+};
+__device__ __forceinline__ Divisor make_divisor(float s) { return Divisor{s, __frcp_rn(s)}; }
+__device__ __forceinline__ float div_rn(float x, const Divisor& d) {
+    float q = x * d.r;
+    q = __fmaf_rn(__fmaf_rn(-d.s, q, x), d.r, q);
+    q = __fmaf_rn(__fmaf_rn(-d.s, q, x), d.r, q);
+    return q;
+}
 
 // thread layout inside a CTA: 16 threads per token row (16 B = 8 channels each), 16 rows per pass
 struct Tile {
@@ -43,25 +58,26 @@ __device__ __forceinline__ float amax8(const uint4& u) {
     return m;
 }
 
-__device__ __forceinline__ uint2 quant8(const uint4& u, float s) {
+__device__ __forceinline__ uint2 quant8(const uint4& u, const Divisor& s) {
     const uint32_t w[4] = {u.x, u.y, u.z, u.w};
     float f[8];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        f[2 * i] = __fdiv_rn(bf16_bits_to_float(w[i] & 0xffffu), s);
-        f[2 * i + 1] = __fdiv_rn(bf16_bits_to_float(w[i] >> 16), s);
+        f[2 * i] = div_rn(bf16_bits_to_float(w[i] & 0xffffu), s);
+        f[2 * i + 1] = div_rn(bf16_bits_to_float(w[i] >> 16), s);
     }
     return make_uint2(cvt4_e4m3(f[0], f[1], f[2], f[3]), cvt4_e4m3(f[4], f[5], f[6], f[7]));
 }
 
-// grid: (nsb, H, 2*B)  blockIdx.z = 2*b + which (0: Q, 1: K)
+// grid: (H, nsb, 2*B), heads fastest so that the CTAs in flight together cover whole 128-token
+// slabs of the [N][H][d] tensor (contiguous DRAM pages); blockIdx.z = 2*b + which (0: Q, 1: K)
 __global__ void __launch_bounds__(QT)
 qk_quantize_kernel(const uint16_t* __restrict__ Q, const uint16_t* __restrict__ K,
                    chorus_attn_shape s, uint8_t* __restrict__ q8, uint8_t* __restrict__ k8,
                    float* __restrict__ q_scale, float* __restrict__ k_scale, int nsb) {
     __shared__ float s_red[QT / 32];
     __shared__ float s_scale;
-    const int blk = blockIdx.x, h = blockIdx.y, b = blockIdx.z >> 1, which = blockIdx.z & 1;
+    const int blk = blockIdx.y, h = blockIdx.x, b = blockIdx.z >> 1, which = blockIdx.z & 1;
     const uint16_t* X = which ? K : Q;
     const int64_t sb = which ? s.k_stride_b : s.q_stride_b;
     const int64_t sn = which ? s.k_stride_n : s.q_stride_n;
@@ -93,7 +109,7 @@ qk_quantize_kernel(const uint16_t* __restrict__ Q, const uint16_t* __restrict__ 
         S[(static_cast<int64_t>(b) * s.H + h) * nsb + blk] = sc;
     }
     __syncthreads();
-    const float sc = s_scale;
+    const Divisor sc = make_divisor(s_scale);
 #pragma unroll
     for (int p = 0; p < 8; ++p) {
         const int n = blk * 128 + p * 16 + rowp;
@@ -104,15 +120,15 @@ qk_quantize_kernel(const uint16_t* __restrict__ Q, const uint16_t* __restrict__ 
     }
 }
 
-// V column amax: grid (chunks, H, B); each CTA covers V_ROWS tokens; atomicMax on float bits
+// V column amax: grid (H, chunks, B); each CTA covers V_ROWS tokens; atomicMax on float bits
 constexpr int V_ROWS = 512;
 __global__ void __launch_bounds__(QT)
 v_amax_kernel(const uint16_t* __restrict__ V, chorus_attn_shape s, float* __restrict__ v_amax) {
     __shared__ float s_m[16][128];
-    const int h = blockIdx.y, b = blockIdx.z;
+    const int h = blockIdx.x, b = blockIdx.z;
     const int sub = threadIdx.x & 15, rowp = threadIdx.x >> 4;
     float m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    const int n0 = blockIdx.x * V_ROWS;
+    const int n0 = blockIdx.y * V_ROWS;
     for (int n = n0 + rowp; n < n0 + V_ROWS && n < s.N; n += 16) {
         const uint4 u = __ldg(reinterpret_cast<const uint4*>(V + b * s.v_stride_b + n * s.v_stride_n +
                                                              h * s.v_stride_h) + sub);
@@ -140,13 +156,13 @@ v_amax_kernel(const uint16_t* __restrict__ V, chorus_attn_shape s, float* __rest
 __global__ void __launch_bounds__(QT)
 v_quantize_kernel(const uint16_t* __restrict__ V, chorus_attn_shape s,
                   const float* __restrict__ v_amax, uint8_t* __restrict__ v8) {
-    const int h = blockIdx.y, b = blockIdx.z;
+    const int h = blockIdx.x, b = blockIdx.z;
     const int sub = threadIdx.x & 15, rowp = threadIdx.x >> 4;
-    float sc[8];
+    Divisor sc[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i)
-        sc[i] = scale_from_amax(v_amax[(static_cast<int64_t>(b) * s.H + h) * 128 + sub * 8 + i]);
-    const int n0 = blockIdx.x * V_ROWS;
+        sc[i] = make_divisor(scale_from_amax(v_amax[(static_cast<int64_t>(b) * s.H + h) * 128 + sub * 8 + i]));
+    const int n0 = blockIdx.y * V_ROWS;
     for (int n = n0 + rowp; n < n0 + V_ROWS && n < s.N; n += 16) {
         const uint4 u = __ldg(reinterpret_cast<const uint4*>(V + b * s.v_stride_b + n * s.v_stride_n +
                                                              h * s.v_stride_h) + sub);
@@ -154,8 +170,8 @@ v_quantize_kernel(const uint16_t* __restrict__ V, chorus_attn_shape s,
         float f[8];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            f[2 * i] = __fdiv_rn(bf16_bits_to_float(w[i] & 0xffffu), sc[2 * i]);
-            f[2 * i + 1] = __fdiv_rn(bf16_bits_to_float(w[i] >> 16), sc[2 * i + 1]);
+            f[2 * i] = div_rn(bf16_bits_to_float(w[i] & 0xffffu), sc[2 * i]);
+            f[2 * i + 1] = div_rn(bf16_bits_to_float(w[i] >> 16), sc[2 * i + 1]);
         }
         uint8_t* dst = v8 + ((static_cast<int64_t>(b) * s.N + n) * s.H + h) * 128;
         reinterpret_cast<uint2*>(dst)[sub] =
@@ -178,9 +194,9 @@ cudaError_t launch_quantize_fp8(const void* Q, const void* K, const void* V,
     const int nv = s.B * s.H * 128;
     cudaError_t e = cudaMemsetAsync(v_scale, 0, sizeof(float) * nv, stream);
     if (e != cudaSuccess) return e;
-    const dim3 gv((s.N + V_ROWS - 1) / V_ROWS, s.H, s.B);
+    const dim3 gv(s.H, (s.N + V_ROWS - 1) / V_ROWS, s.B);
     v_amax_kernel<<<gv, QT, 0, stream>>>(static_cast<const uint16_t*>(V), s, v_scale);
-    qk_quantize_kernel<<<dim3(nsb, s.H, 2 * s.B), QT, 0, stream>>>(
+    qk_quantize_kernel<<<dim3(s.H, nsb, 2 * s.B), QT, 0, stream>>>(
         static_cast<const uint16_t*>(Q), static_cast<const uint16_t*>(K), s,
         static_cast<uint8_t*>(q8), static_cast<uint8_t*>(k8), q_scale, k_scale, nsb);
     v_quantize_kernel<<<gv, QT, 0, stream>>>(static_cast<const uint16_t*>(V), s, v_scale,
