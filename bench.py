@@ -59,31 +59,57 @@ def attn_flops(cfg, density):
 # clock sampling during the timed region
 # --------------------------------------------------------------------------------------------------
 class ClockSampler:
+    """SM clock and throttle reasons sampled DURING the timed region: NVML every 2 ms when the
+    nvidia_ml_py binding is there (the timed region is only ~0.2 s), else `nvidia-smi` every 0.1 s."""
     QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
              "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
-    def __init__(self, index: int):
+    def __init__(self, index: int, uuid: str | None = None):
         self.index = index
-        self.samples = []
+        self.samples = []          # (sm_mhz, sm_max_mhz, [active reason names])
         self._stop = threading.Event()
         self._thr = None
+        self._nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            # CUDA ordinals follow CUDA_VISIBLE_DEVICES, NVML's do not: go by UUID when torch gives one
+            self._h = (pynvml.nvmlDeviceGetHandleByUUID(uuid) if uuid
+                       else pynvml.nvmlDeviceGetHandleByIndex(index))
+            self._max = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+            self._bits = [(pynvml.nvmlClocksEventReasonHwSlowdown, "hw_slowdown"),
+                          (pynvml.nvmlClocksEventReasonHwThermalSlowdown, "hw_thermal_slowdown"),
+                          (pynvml.nvmlClocksEventReasonSwThermalSlowdown, "sw_thermal_slowdown"),
+                          (pynvml.nvmlClocksEventReasonSwPowerCap, "sw_power_cap")]
+            self._nvml = pynvml
+        except Exception:
+            self._nvml = None
 
     def _sample_once(self):
         try:
+            if self._nvml is not None:
+                n = self._nvml
+                mhz = float(n.nvmlDeviceGetClockInfo(self._h, n.NVML_CLOCK_SM))
+                mask = int(n.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                self.samples.append((mhz, self._max, [nm for bit, nm in self._bits if mask & bit]))
+                return
             out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}",
                                   "--format=csv,noheader,nounits"], capture_output=True, text=True,
                                  timeout=5).stdout.strip().splitlines()
             if out:
                 f = [x.strip() for x in out[0].split(",")]
-                self.samples.append((float(f[0]), float(f[1]), f[3:]))
+                self.samples.append((float(f[0]), float(f[1]),
+                                     [n for n, v in zip(self.NAMES, f[3:]) if v.lower().startswith("active")]))
         except Exception:
             pass
 
     def _run(self):
+        period = 0.002 if self._nvml is not None else 0.1
         while not self._stop.is_set():
             self._sample_once()
-            self._stop.wait(0.1)
+            self._stop.wait(period)
 
     def start(self):
         self._thr = threading.Thread(target=self._run, daemon=True)
@@ -95,10 +121,11 @@ class ClockSampler:
             self._thr.join(timeout=10)
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({n for _, _, fl in self.samples for n, v in zip(names, fl) if v.lower().startswith("active")})
+        reasons = sorted({n for _, _, fl in self.samples for n in fl})
         return {"sm_mhz": statistics.median(s[0] for s in self.samples),
-                "sm_max_mhz": self.samples[0][1], "reasons": reasons, "samples": len(self.samples)}
+                "sm_min_mhz": min(s[0] for s in self.samples),
+                "sm_max_mhz": self.samples[0][1], "reasons": reasons, "samples": len(self.samples),
+                "via": "nvml" if self._nvml is not None else "nvidia-smi"}
 
 
 # --------------------------------------------------------------------------------------------------
@@ -237,7 +264,11 @@ def run_chorus(args):
     for _ in range(args.warmup):
         step()
     barrier()
-    sampler = ClockSampler(local)
+    try:
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(local).uuid)
+    except Exception:
+        uuid = None
+    sampler = ClockSampler(local, uuid)
     if rank == 0:
         sampler.start()
     K = args.steps
@@ -276,6 +307,31 @@ def run_chorus(args):
     barrier()
     e2e_ms = a.elapsed_time(b_) / e2e_steps
     clocks = sampler.stop() if rank == 0 else None
+
+    # mask decode at the size where it is HBM-bound: a whole stored mask set (40 layers x H heads,
+    # SURVEY section 8 d-4), timed alone with a flushed L2; reported beside the per-layer figure
+    set_ms = set_bytes = None
+    if rank == 0 and cfg.name.startswith("cfg2"):
+        Lset = 40
+        dMs = dM.repeat(Lset, 1, 1, 1).contiguous()
+        rows_s = Lset * rows
+        rp_s = torch.empty(rows_s + 1, dtype=torch.int32, device=dev)
+        ci_s = torch.empty(int(density * rows_s * cfg.nk) + 1024, dtype=torch.int32, device=dev)
+        ws_s = torch.empty(max(4, B.mask_to_index_workspace_bytes(Lset, cfg.H, cfg.nq, cfg.nk)), dtype=torch.uint8, device=dev)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        ts = []
+        for i in range(8):
+            flush.zero_()
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            B.chorus_mask_to_index(dMs, cfg.nk, row_ptr=rp_s, col_idx=ci_s, workspace=ws_s)
+            b_.record(stream)
+            torch.cuda.synchronize()
+            if i >= 3:
+                ts.append(a.elapsed_time(b_))
+        set_ms = statistics.median(ts)
+        set_bytes = 4 * rows_s * cfg.words + 4 * (rows_s + 1) + 4 * int(rp_s[-1].item())
+        del dMs, rp_s, ci_s, flush
 
     t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
     if world > 1:
@@ -318,11 +374,18 @@ def run_chorus(args):
                           "attn_bf16_ms": attn_ms, "attn_bf16_TFLOPs": achieved,
                           "routing_overhead_ratio": dec_ms / (dec_ms + attn_ms)},
         }
+        if set_ms is not None:
+            line["breakdown"].update({"decode_set_ms": set_ms, "decode_set_bytes": set_bytes,
+                                      "decode_set_GBps": set_bytes / (set_ms * 1e-3) / 1e9,
+                                      "decode_set_frac_of_hbm": set_bytes / (set_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                      "decode_set": "40 layers x %d heads x %d rows, L2 flushed, median of 5" % (cfg.H, cfg.nq)})
         if has_fp8:
             a8 = flops_attn / (attn8_ms * 1e-3) / 1e12
             line["breakdown"].update({"quantize_ms": quant_ms, "attn_fp8_ms": attn8_ms, "attn_fp8_TFLOPs": a8,
                                       "attn_fp8_frac_of_2x_bf16_peak": a8 / (2 * peaks["bf16"]),
-                                      "attn_fp8_frac_of_datasheet_4500": a8 / 4500.0})
+                                      "attn_fp8_frac_of_datasheet_4500": a8 / 4500.0,
+                                      "attn_fp8_traffic": json.load(open(tp)).get(f"{cfg.name}_fp8_attn_dram_bytes_per_launch")
+                                      if os.path.exists(tp) else None})
         if world == 1 and not args.no_cpu_baseline:
             heads = min(cfg.H, 4)
             line["cpu_baseline"] = cpu_baseline(W.scaled(cfg, H=heads), Qb[:, :, :heads].copy(),
