@@ -153,3 +153,39 @@ def visit_refresh(mask, nk, group=8):
     L, H, nq, words = m.shape
     lib().oracle_visit_refresh(_p(m), L, H, nq, nk, group)
     return m
+
+
+def block_mass(Q, K, scale, n_threads=0):
+    """True (dense) attention mass per block pair: Q, K bf16-bit arrays
+    [B][N][H][d] -> float64 [B][H][nq][nk]; every valid query row contributes exactly 1."""
+    assert Q.dtype == K.dtype == np.uint16
+    B, N, H, d = Q.shape
+    nq, nk = (N + BQ - 1) // BQ, (N + BK - 1) // BK
+    out = np.zeros((B, H, nq, nk), dtype=np.float64)
+    lib().oracle_block_mass(_p(Q), _p(K), B, H, N, d, *_strides(Q), *_strides(K),
+                            C.c_double(scale), _p(out), C.c_int(n_threads))
+    return out
+
+
+def mask_from_mass(mass, nk, top_p, min_top_k):
+    """Top-p with a top-k floor (PAPER.md:L81, L93 (2)): mass float32 [..., nk] -> (bitmask uint32
+    [..., words], kept int32 [...])."""
+    m = _c(mass, np.float32)
+    assert m.shape[-1] == nk
+    rows = m.size // nk
+    words = (nk + 31) // 32
+    bm = np.zeros(m.shape[:-1] + (words,), dtype=np.uint32)
+    kept = np.zeros(m.shape[:-1], dtype=np.int32)
+    lib().oracle_mask_from_mass(_p(m), C.c_int64(rows), nk, C.c_double(top_p), C.c_double(min_top_k),
+                                _p(bm), _p(kept))
+    return bm, kept
+
+
+def mask_coverage(mass, bitmask, nk):
+    """Per-head coverage: mass float32 [heads][nq][nk], bitmask [heads][nq][words]."""
+    m = _c(mass, np.float32)
+    b = _c(bitmask, np.uint32)
+    heads, nq = m.shape[0], m.shape[1]
+    out = np.zeros(heads, dtype=np.float64)
+    lib().oracle_mask_coverage(_p(m), _p(b), heads, nq, nk, _p(out))
+    return out

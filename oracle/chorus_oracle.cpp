@@ -22,6 +22,11 @@
 //                               by the paper and pinned only by BASELINE.json cfg3.
 //   oracle_retrieve_top1        pinned (planted neighbour, numpy argmax)
 //   oracle_visit_refresh        pinned (brute force per bit, every pair visited once per group)
+//   oracle_block_mass           pinned (numpy dense softmax summed per block, rows sum to 1, uniform
+//                               attention closed form)
+//   oracle_mask_from_mass       pinned (exact-rational brute force on tiny rows, minimality of the
+//                               kept prefix, floor count, ties by index, hand-worked golden row)
+//   oracle_mask_coverage        pinned (numpy; full mask = 1, top-p mask >= p)
 //
 // Build: g++ -O3 -march=native -fopenmp -shared -fPIC (see oracle/build.py).
 
@@ -346,6 +351,121 @@ void oracle_visit_refresh(uint32_t* mask, int L, int H, int nq, int nk, int grou
                     }
                 }
             }
+    }
+}
+
+// -------------------------------------------------------------------------------------------------
+// Mask construction from a dense pass ("in the dense case we select a block-level mask
+// from its attention map via top-p with a top-k floor"; L73 "coverage: the fraction of the target's
+// true token-level attention mass that falls within the blocks it selects"; L93 (2) min_top_k: "every
+// head retains at least a fraction k_min of its key blocks"; L153 defaults top_p 0.95 / 0.9,
+// min_top_k 0.1 / 0.0).  Readings R21-R23 in DESIGN.md section 3.
+// -------------------------------------------------------------------------------------------------
+
+// Block mass of the TRUE (dense) attention: mass[h][qb][kb] = sum over queries i of q-block qb and
+// keys j of k-block kb of softmax_j(scale * q_i . k_j), all N keys retained, fp64, two-pass softmax.
+// Q, K: bf16 bits [B][N][H][d] (element strides); mass: double [B][H][nq][nk].  Each row of a
+// q-block contributes exactly 1, so a q-block's masses sum to its number of valid rows.
+void oracle_block_mass(const uint16_t* Q, const uint16_t* K, int B, int H, int N, int d,
+                       int64_t q_sb, int64_t q_sn, int64_t q_sh, int64_t k_sb, int64_t k_sn,
+                       int64_t k_sh, double scale, double* mass, int n_threads) {
+    const int nq = (N + 127) / 128, nk = (N + 63) / 64;
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+    const int64_t total = static_cast<int64_t>(B) * H * nq;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t it = 0; it < total; ++it) {
+        const int qb = static_cast<int>(it % nq);
+        const int h = static_cast<int>((it / nq) % H);
+        const int b = static_cast<int>(it / (static_cast<int64_t>(nq) * H));
+        double* out = mass + it * nk;
+        for (int kb = 0; kb < nk; ++kb) out[kb] = 0.0;
+        std::vector<double> kd(static_cast<size_t>(N) * d), s(N), q(d);
+        for (int j = 0; j < N; ++j)
+            for (int c = 0; c < d; ++c) kd[static_cast<size_t>(j) * d + c] = bf16_to_double(K[b * k_sb + j * k_sn + h * k_sh + c]);
+        for (int i = qb * 128; i < N && i < qb * 128 + 128; ++i) {
+            for (int c = 0; c < d; ++c) q[c] = bf16_to_double(Q[b * q_sb + i * q_sn + h * q_sh + c]);
+            double m = -std::numeric_limits<double>::infinity();
+            for (int j = 0; j < N; ++j) {
+                double acc = 0.0;
+                for (int c = 0; c < d; ++c) acc += q[c] * kd[static_cast<size_t>(j) * d + c];
+                s[j] = scale * acc;
+                if (s[j] > m) m = s[j];
+            }
+            double l = 0.0;
+            for (int j = 0; j < N; ++j) {
+                s[j] = std::exp(s[j] - m);
+                l += s[j];
+            }
+            for (int j = 0; j < N; ++j) out[j / 64] += s[j] / l;
+        }
+    }
+}
+
+// Top-p with a top-k floor, one row of nk block masses at a time (R22): the masses (fp32, >= 0) are
+// taken in units of 2^-24 (q = floor(mass * 2^24), an exact integer), so that sums do not depend on
+// the order of addition; blocks are ranked by q descending, ties by index ascending; the row keeps
+// the shortest prefix of that ranking whose q-sum reaches ceil(top_p * total q), and never fewer
+// than ceil(min_top_k * nk) blocks.  A row without any mass keeps only the floor.
+// mass: float [rows][nk] -> bitmask uint32 [rows][words] (pad bits 0), kept[rows] = blocks kept.
+void oracle_mask_from_mass(const float* mass, int64_t rows, int nk, double top_p, double min_top_k,
+                           uint32_t* bitmask, int32_t* kept) {
+    const int words = (nk + 31) / 32;
+    int n_floor = static_cast<int>(std::ceil(min_top_k * static_cast<double>(nk)));
+    if (n_floor < 0) n_floor = 0;
+    if (n_floor > nk) n_floor = nk;
+    std::vector<uint64_t> q(nk);
+    std::vector<int> order(nk);
+    for (int64_t r = 0; r < rows; ++r) {
+        const float* mr = mass + r * nk;
+        uint64_t total = 0;
+        for (int k = 0; k < nk; ++k) {
+            q[k] = static_cast<uint64_t>(std::floor(static_cast<double>(mr[k]) * 16777216.0));
+            total += q[k];
+            order[k] = k;
+        }
+        // selection sort into (q descending, index ascending): plain and obviously right
+        for (int a = 0; a < nk; ++a) {
+            int best = a;
+            for (int c = a + 1; c < nk; ++c) {
+                const int x = order[c], y = order[best];
+                if (q[x] > q[y] || (q[x] == q[y] && x < y)) best = c;
+            }
+            const int t = order[a];
+            order[a] = order[best];
+            order[best] = t;
+        }
+        const uint64_t target = static_cast<uint64_t>(std::ceil(top_p * static_cast<double>(total)));
+        int n_p = 0;
+        if (total > 0) {
+            uint64_t acc = 0;
+            while (n_p < nk && acc < target) acc += q[order[n_p++]];
+        }
+        const int n = n_p > n_floor ? n_p : n_floor;
+        uint32_t* br = bitmask + r * words;
+        for (int w = 0; w < words; ++w) br[w] = 0u;
+        for (int a = 0; a < n; ++a) br[order[a] >> 5] |= (1u << (order[a] & 31));
+        if (kept) kept[r] = n;
+    }
+}
+
+// Coverage of a mask on a mass map, per head: sum of the masses of the kept blocks
+// over the sum of all masses.  mass: float [heads][nq][nk], bitmask [heads][nq][words].
+void oracle_mask_coverage(const float* mass, const uint32_t* bitmask, int heads, int nq, int nk,
+                          double* coverage) {
+    const int words = (nk + 31) / 32;
+    for (int h = 0; h < heads; ++h) {
+        double in = 0.0, all = 0.0;
+        for (int qb = 0; qb < nq; ++qb) {
+            const int64_t r = static_cast<int64_t>(h) * nq + qb;
+            for (int kb = 0; kb < nk; ++kb) {
+                const double m = static_cast<double>(mass[r * nk + kb]);
+                all += m;
+                if (mask_bit(bitmask + r * words, kb)) in += m;
+            }
+        }
+        coverage[h] = all > 0.0 ? in / all : 0.0;
     }
 }
 
