@@ -167,6 +167,45 @@ chorus_status chorus_retrieve_top1(const float* bank, int n, int dim, const floa
                                    int32_t* best_idx, float* best_sim, int32_t* hit,
                                    void* workspace, size_t* workspace_bytes, void* cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Mask construction from a dense pass (the historical request's side of sparsity reuse,
+ * "in the dense case we select a block-level mask from its attention map via top-p
+ * with a top-k floor"; L93 (2) min_top_k; L73 coverage; defaults at L153: top_p 0.95 / 0.9,
+ * min_top_k 0.1 / 0.0).  Three calls: block mass -> mask -> (optionally) coverage.
+ *
+ * chorus_block_mass: mass[b][h][qb][kb] = sum over queries i of query block qb and keys j of key
+ *   block kb of softmax_j(scale * <Q[i], K[j]>), the softmax taken over ALL N keys (the true, dense
+ *   attention).  Every valid query row contributes exactly 1.
+ *   Q, K     device, bf16, [B][N][H][d] with the q_/k_ strides of `shape` (v_/o_ strides ignored);
+ *            16-byte aligned, strides multiples of 8 elements, d = 128.
+ *   mass     device, float [B][H][ceil(N/128)][ceil(N/64)], fully overwritten.
+ *   Accuracy against the fp64 oracle: |err| <= 2e-3 * max(mass, 1e-3) + 1e-5 per block (bf16
+ *   products, fp32 sums, ex2.approx); the result is deterministic (fixed summation order).
+ *
+ * chorus_mask_from_mass: one row of nk_blk masses at a time (R22): masses are taken in
+ *   units of 2^-24 (q = floor(mass * 2^24)), ranked by q descending with ties by index ascending;
+ *   the row keeps the shortest prefix whose q-sum reaches ceil(top_p * sum q) (double product) and
+ *   never fewer than ceil(min_top_k * nk_blk) blocks (double product).  Integer decisions: the
+ *   result is compared bit-exactly with the oracle on the same masses.
+ *   mass     device, float [rows][nk_blk], finite and >= 0;  nk_blk <= 2048.
+ *   bitmask  device, uint32 [rows][ceil(nk_blk/32)], fully overwritten, pad bits 0 (the layout
+ *            chorus_mask_to_index reads).
+ *   kept     device, int32 [rows] or NULL: number of blocks kept per row.
+ *
+ * chorus_mask_coverage: coverage[h] = sum of the masses of the kept blocks of head h / sum of all
+ *   its masses (0 if a head has no mass); fp64 accumulation, fixed order.
+ *   mass [heads][nq_blk][nk_blk] float, bitmask [heads][nq_blk][words], coverage float [heads].
+ * Errors: INVALID_ARG (null, sizes <= 0, top_p / min_top_k outside [0, 1], misalignment),
+ *         UNSUPPORTED (d != 128, nk_blk > 2048), CUDA.
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
+                                const chorus_attn_shape* shape, float* mass, void* cuda_stream);
+chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk, float top_p,
+                                    float min_top_k, uint32_t* bitmask, int32_t* kept,
+                                    void* cuda_stream);
+chorus_status chorus_mask_coverage(const float* mass, const uint32_t* bitmask, int heads, int nq_blk,
+                                   int nk_blk, float* coverage, void* cuda_stream);
+
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char* chorus_last_error(void);
 

@@ -155,15 +155,17 @@ def visit_refresh(mask, nk, group=8):
     return m
 
 
-def block_mass(Q, K, scale, n_threads=0):
+def block_mass(Q, K, scale, qblocks=None, n_threads=0):
     """True (dense) attention mass per block pair: Q, K bf16-bit arrays
-    [B][N][H][d] -> float64 [B][H][nq][nk]; every valid query row contributes exactly 1."""
+    [B][N][H][d] -> float64 [B][H][nq][nk]; every valid query row contributes exactly 1.
+    qblocks: only these query blocks are computed (the rest of the output is 0)."""
     assert Q.dtype == K.dtype == np.uint16
     B, N, H, d = Q.shape
     nq, nk = (N + BQ - 1) // BQ, (N + BK - 1) // BK
     out = np.zeros((B, H, nq, nk), dtype=np.float64)
+    sel = _c(np.asarray([] if qblocks is None else qblocks), np.int32)
     lib().oracle_block_mass(_p(Q), _p(K), B, H, N, d, *_strides(Q), *_strides(K),
-                            C.c_double(scale), _p(out), C.c_int(n_threads))
+                            C.c_double(scale), _p(out), C.c_int(sel.size), _p(sel), C.c_int(n_threads))
     return out
 
 

@@ -368,7 +368,9 @@ void oracle_visit_refresh(uint32_t* mask, int L, int H, int nq, int nk, int grou
 // q-block contributes exactly 1, so a q-block's masses sum to its number of valid rows.
 void oracle_block_mass(const uint16_t* Q, const uint16_t* K, int B, int H, int N, int d,
                        int64_t q_sb, int64_t q_sn, int64_t q_sh, int64_t k_sb, int64_t k_sn,
-                       int64_t k_sh, double scale, double* mass, int n_threads) {
+                       int64_t k_sh, double scale, double* mass, int n_sel, const int32_t* sel_qb,
+                       int n_threads) {
+    // n_sel > 0: only the query blocks listed in sel_qb are computed (the others stay as they are)
     const int nq = (N + 127) / 128, nk = (N + 63) / 64;
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
@@ -379,6 +381,11 @@ void oracle_block_mass(const uint16_t* Q, const uint16_t* K, int B, int H, int N
         const int qb = static_cast<int>(it % nq);
         const int h = static_cast<int>((it / nq) % H);
         const int b = static_cast<int>(it / (static_cast<int64_t>(nq) * H));
+        if (n_sel > 0) {
+            bool wanted = false;
+            for (int t = 0; t < n_sel; ++t) wanted = wanted || sel_qb[t] == qb;
+            if (!wanted) continue;
+        }
         double* out = mass + it * nk;
         for (int kb = 0; kb < nk; ++kb) out[kb] = 0.0;
         std::vector<double> kd(static_cast<size_t>(N) * d), s(N), q(d);

@@ -19,7 +19,8 @@ CHORUS_BF16, CHORUS_FP8_E4M3 = 0, 1
 BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
 
 EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
-           "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_last_error", "chorus_version",
+           "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
+           "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count"]
 
 
@@ -65,6 +66,12 @@ def lib() -> C.CDLL:
         L.chorus_retrieve_top1.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_float,
                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.POINTER(C.c_size_t), C.c_void_p]
+        L.chorus_block_mass.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.POINTER(AttnShape),
+                                        C.c_void_p, C.c_void_p]
+        L.chorus_mask_from_mass.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_float, C.c_float,
+                                            C.c_void_p, C.c_void_p, C.c_void_p]
+        L.chorus_mask_coverage.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
+                                           C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -208,3 +215,42 @@ def chorus_retrieve_top1(bank, query, tau: float, out=None, workspace=None, stre
                                       _ptr(out[1]), _ptr(out[2]), _ptr(workspace), C.byref(wsb),
                                       _stream(stream)))
     return out
+
+
+def chorus_block_mass(Q, K, scale: float, mass=None, stream=None):
+    """bf16 Q, K [B][N][H][d] (cuda) -> float32 mass [B][H][ceil(N/128)][ceil(N/64)] of the dense
+    attention (PAPER.md:L73, L81)."""
+    B, N, H, d = Q.shape
+    nq, nk = (N + BLOCK_Q - 1) // BLOCK_Q, (N + BLOCK_K - 1) // BLOCK_K
+    if mass is None:
+        mass = torch.empty((B, H, nq, nk), dtype=torch.float32, device=Q.device)
+    shape = attn_shape(Q, K, K)
+    _check(lib().chorus_block_mass(_ptr(Q), _ptr(K), C.c_float(scale), C.byref(shape), _ptr(mass),
+                                   _stream(stream)))
+    return mass
+
+
+def chorus_mask_from_mass(mass, top_p: float, min_top_k: float, bitmask=None, kept=None, stream=None):
+    """float32 mass [..., nk] (cuda) -> (bitmask int32-bits [..., ceil(nk/32)], kept int32 [...]):
+    top-p with a top-k floor (PAPER.md:L81, L93 (2))."""
+    assert mass.is_cuda and mass.is_contiguous() and mass.dtype == torch.float32
+    nk = mass.shape[-1]
+    rows = mass.numel() // nk
+    if bitmask is None:
+        bitmask = torch.empty(mass.shape[:-1] + ((nk + 31) // 32,), dtype=torch.int32, device=mass.device)
+    if kept is None:
+        kept = torch.empty(mass.shape[:-1], dtype=torch.int32, device=mass.device)
+    _check(lib().chorus_mask_from_mass(_ptr(mass), rows, nk, C.c_float(top_p), C.c_float(min_top_k),
+                                       _ptr(bitmask), _ptr(kept), _stream(stream)))
+    return bitmask, kept
+
+
+def chorus_mask_coverage(mass, bitmask, nk_blk: int, coverage=None, stream=None):
+    """mass float32 [heads][nq][nk], bitmask [heads][nq][words] (cuda) -> float32 coverage [heads]."""
+    heads, nq, nk = mass.shape
+    assert nk == nk_blk and mass.is_contiguous() and bitmask.is_contiguous()
+    if coverage is None:
+        coverage = torch.empty(heads, dtype=torch.float32, device=mass.device)
+    _check(lib().chorus_mask_coverage(_ptr(mass), _ptr(bitmask), heads, nq, nk, _ptr(coverage),
+                                      _stream(stream)))
+    return coverage

@@ -215,6 +215,51 @@ chorus_status chorus_block_sparse_attn_fwd(const void* Q, const void* K, const v
     return check_cuda(e, "attention launch");
 }
 
+chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
+                                const chorus_attn_shape* shape, float* mass, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!Q || !K || !mass) return set_error(CHORUS_ERR_INVALID_ARG, "Q, K, mass must be non-null");
+    if (!aligned16(Q) || !aligned16(K)) return set_error(CHORUS_ERR_INVALID_ARG, "Q, K must be 16-byte aligned");
+    if (!shape) return set_error(CHORUS_ERR_INVALID_ARG, "shape is null");
+    // only the q_ / k_ strides are used: validate a copy whose v_ strides repeat k_
+    chorus_attn_shape s = *shape;
+    s.v_stride_b = s.k_stride_b; s.v_stride_n = s.k_stride_n; s.v_stride_h = s.k_stride_h;
+    chorus_status st = validate_shape(&s, 8, false);
+    if (st != CHORUS_OK) return st;
+    CUtensorMap tmQ, tmK;
+    if ((st = make_tmap(&tmQ, Q, 2, s.B, s.H, s.N, s.d, s.q_stride_b, s.q_stride_n, s.q_stride_h,
+                        64, 128, "Q")) != CHORUS_OK) return st;
+    if ((st = make_tmap(&tmK, K, 2, s.B, s.H, s.N, s.d, s.k_stride_b, s.k_stride_n, s.k_stride_h,
+                        64, 128, "K")) != CHORUS_OK) return st;
+    return check_cuda(launch_block_mass(tmQ, tmK, mass, s.B, s.H, s.N, scale * 1.4426950408889634f,
+                                        static_cast<cudaStream_t>(cuda_stream)), "block mass launch");
+}
+
+chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk, float top_p,
+                                    float min_top_k, uint32_t* bitmask, int32_t* kept,
+                                    void* cuda_stream) {
+    g_err[0] = 0;
+    if (!mass || !bitmask) return set_error(CHORUS_ERR_INVALID_ARG, "mass / bitmask is null");
+    if (rows <= 0 || nk_blk <= 0) return set_error(CHORUS_ERR_INVALID_ARG, "rows, nk_blk must be positive");
+    if (rows > INT32_MAX) return set_error(CHORUS_ERR_CAPACITY, "rows = %lld exceeds INT32_MAX", (long long)rows);
+    if (nk_blk > 2048) return set_error(CHORUS_ERR_UNSUPPORTED, "nk_blk = %d > 2048", nk_blk);
+    if (!(top_p >= 0.f && top_p <= 1.f) || !(min_top_k >= 0.f && min_top_k <= 1.f))
+        return set_error(CHORUS_ERR_INVALID_ARG, "top_p and min_top_k must lie in [0, 1]");
+    return check_cuda(launch_mask_from_mass(mass, rows, nk_blk, static_cast<double>(top_p),
+                                            static_cast<double>(min_top_k), bitmask, kept,
+                                            static_cast<cudaStream_t>(cuda_stream)), "mask_from_mass launch");
+}
+
+chorus_status chorus_mask_coverage(const float* mass, const uint32_t* bitmask, int heads, int nq_blk,
+                                   int nk_blk, float* coverage, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!mass || !bitmask || !coverage) return set_error(CHORUS_ERR_INVALID_ARG, "mass / bitmask / coverage is null");
+    if (heads <= 0 || nq_blk <= 0 || nk_blk <= 0)
+        return set_error(CHORUS_ERR_INVALID_ARG, "heads, nq_blk, nk_blk must be positive");
+    return check_cuda(launch_mask_coverage(mass, bitmask, heads, nq_blk, nk_blk, coverage,
+                                           static_cast<cudaStream_t>(cuda_stream)), "mask_coverage launch");
+}
+
 chorus_status chorus_quantize_fp8(const void* Q, const void* K, const void* V,
                                   const chorus_attn_shape* shape, void* q8, void* k8, void* v8,
                                   float* q_scale, float* k_scale, float* v_scale,

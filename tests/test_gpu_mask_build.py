@@ -1,0 +1,120 @@
+"""GPU parity of the mask-construction calls (PAPER.md:L73, L81, L93 (2)): chorus_block_mass against
+the fp64 oracle within the tolerance of include/chorus.h, chorus_mask_from_mass bit-exactly on the
+same masses, chorus_mask_coverage against the oracle, and the three chained at a full-size head."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from gpu_common import dbf16, dev
+from helpers import random_qkv_bits
+from paper_2606_25040_b200 import binding as B
+from paper_2606_25040_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+F = lambda x: float(np.float32(x))      # the ABI takes float: the oracle gets the same value
+
+
+def mass_close(got, ref):
+    tol = 2e-3 * np.maximum(ref, 1e-3) + 1e-5
+    bad = np.abs(got - ref) > tol
+    assert not bad.any(), (int(bad.sum()), float(np.abs(got - ref).max()))
+
+
+@pytest.mark.parametrize("N,H,scale", [(512, 2, 0.0884), (200, 1, 0.3), (1000, 3, 0.0884), (64, 1, 1.0),
+                                        (129, 2, 0.5)])
+def test_block_mass_matches_oracle(N, H, scale):
+    Q, K, _ = random_qkv_bits(N, H, seed=N + H)
+    ref = oracle.block_mass(Q, K, scale)
+    got = B.chorus_block_mass(dbf16(Q), dbf16(K), scale)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy().astype(np.float64)
+    assert got.shape == ref.shape
+    mass_close(got, ref)
+    nq = (N + 127) // 128
+    rows = np.minimum(128, N - 128 * np.arange(nq))
+    assert np.allclose(got.sum(axis=-1), rows[None, None, :], rtol=1e-4)      # one unit per query row
+
+
+def test_block_mass_peaked_rows_and_batch():
+    # large scale: almost all mass on one key per row; two batches; strided [B][H][N][d] storage
+    N, H = 384, 2
+    Q, K, _ = random_qkv_bits(N, H, seed=3, B=2)
+    ref = oracle.block_mass(Q, K, 2.0)
+    q = dbf16(Q).permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3)
+    k = dbf16(K).permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3)
+    got = B.chorus_block_mass(q, k, 2.0)
+    torch.cuda.synchronize()
+    mass_close(got.cpu().numpy().astype(np.float64), ref)
+
+
+def test_block_mass_is_deterministic():
+    N, H = 640, 2
+    Q, K, _ = random_qkv_bits(N, H, seed=9)
+    a = B.chorus_block_mass(dbf16(Q), dbf16(K), 0.2)
+    b = B.chorus_block_mass(dbf16(Q), dbf16(K), 0.2)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("nk", [1, 31, 32, 33, 64, 257, 512, 1182, 2048])
+def test_mask_from_mass_bit_exact(nk):
+    g = np.random.default_rng(nk)
+    rows = 37
+    mass = (g.random((rows, nk)) ** 5).astype(np.float32) * np.float32(128.0)
+    mass[1] = 0.0
+    mass[2, : (nk + 1) // 2] = mass[2, 0]            # ties
+    mass[3] = np.float32(1.0)                        # all equal: index order decides
+    dm = torch.from_numpy(mass).to(dev())
+    for top_p, k_min in ((0.95, 0.1), (0.9, 0.0), (0.5, 0.3), (1.0, 0.0), (0.0, 0.0), (0.0, 1.0)):
+        bm_o, kept_o = oracle.mask_from_mass(mass, nk, F(top_p), F(k_min))
+        bm, kept = B.chorus_mask_from_mass(dm, top_p, k_min)
+        torch.cuda.synchronize()
+        assert np.array_equal(bm.cpu().numpy().view(np.uint32), bm_o), (nk, top_p, k_min)
+        assert np.array_equal(kept.cpu().numpy(), kept_o)
+
+
+def test_mask_coverage_matches_oracle():
+    g = np.random.default_rng(5)
+    H, nq, nk = 5, 7, 100
+    mass = (g.random((H, nq, nk)) ** 3).astype(np.float32)
+    mass[4] = 0.0
+    keep = g.random((H, nq, nk)) < 0.3
+    bm = W.pack_bits(keep)
+    cov = B.chorus_mask_coverage(torch.from_numpy(mass).to(dev()),
+                                 torch.from_numpy(bm.view(np.int32)).to(dev()), nk)
+    torch.cuda.synchronize()
+    assert np.allclose(cov.cpu().numpy(), oracle.mask_coverage(mass, bm, nk), atol=2e-7)
+
+
+def test_true_top_p_mask_of_one_full_size_head():
+    # 480p head (N = 32760, 256 x 512 blocks): mass -> mask -> coverage -> decode, all on the device.
+    # The oracle computes the mass of sampled query blocks only (a full head takes too long).
+    cfg = W.scaled(W.CFG2, H=1)
+    Q, K, _ = W.qkv_bits(cfg)
+    tq, tk = dbf16(Q), dbf16(K)
+    scale = 0.35                                   # N(0,1) data at 1/sqrt(d) is nearly uniform: sharpen it
+    mass = B.chorus_block_mass(tq, tk, scale)
+    torch.cuda.synchronize()
+    m = mass.cpu().numpy()
+    rows = np.minimum(128, cfg.N - 128 * np.arange(cfg.nq))
+    assert np.allclose(m[0, 0].sum(axis=1), rows, rtol=2e-4)
+    sel = [0, 100, cfg.nq - 1]
+    ref = oracle.block_mass(Q, K, scale, qblocks=sel)
+    for qb in sel:
+        mass_close(m[0, 0, qb].astype(np.float64), ref[0, 0, qb])
+    top_p, k_min = 0.9, 0.1
+    bm, kept = B.chorus_mask_from_mass(mass[0], top_p, k_min)
+    bm_o, kept_o = oracle.mask_from_mass(m[0], cfg.nk, F(top_p), F(k_min))
+    torch.cuda.synchronize()
+    assert np.array_equal(bm.cpu().numpy().view(np.uint32), bm_o)
+    cov = B.chorus_mask_coverage(mass[0], bm, cfg.nk).cpu().numpy()
+    assert np.allclose(cov, oracle.mask_coverage(m[0], bm_o, cfg.nk), atol=2e-6)
+    assert (cov >= 0.9 - 1e-5).all()
+    k = kept.cpu().numpy()
+    assert k.min() >= int(np.ceil(F(k_min) * cfg.nk)) and k.max() <= cfg.nk
+    # the mask feeds the reuse path unchanged
+    rp, ci = B.chorus_mask_to_index(bm[None], cfg.nk)
+    rp_o, ci_o = oracle.mask_to_index(bm_o[None], cfg.nk)
+    assert np.array_equal(rp.cpu().numpy(), rp_o) and np.array_equal(ci.cpu().numpy()[: len(ci_o)], ci_o)
