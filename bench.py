@@ -201,6 +201,24 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------------------------------
+# multi-rank aggregation ("replicas only": no data-path collective; only the timings are reduced)
+# --------------------------------------------------------------------------------------------------
+def max_over_ranks(values, device, world):
+    """Device-side times of all ranks -> the slowest rank's (the driver's contract: max over ranks)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def whole_job_value(world, flops_per_rank_step, ms_per_step):
+    """Aggregate TFLOP/s of `world` replicas that each do flops_per_rank_step in ms_per_step (max)."""
+    return world * flops_per_rank_step / (ms_per_step * 1e-3) / 1e12
+
+
+# --------------------------------------------------------------------------------------------------
 # the CUDA path
 # --------------------------------------------------------------------------------------------------
 def run_chorus(args):
@@ -333,14 +351,11 @@ def run_chorus(args):
         set_bytes = 4 * rows_s * cfg.words + 4 * (rows_s + 1) + 4 * int(rp_s[-1].item())
         del dMs, rp_s, ci_s, flush
 
-    t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = t.tolist()
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], dev, world)
     ms_per_step = total_ms / K
     step_flops = flops_attn * (2 if has_fp8 else 1)
-    value = world * step_flops / (ms_per_step * 1e-3) / 1e12
-    e2e_val = world * step_flops / (e2e_ms * 1e-3) / 1e12
+    value = whole_job_value(world, step_flops, ms_per_step)
+    e2e_val = whole_job_value(world, step_flops, e2e_ms)
 
     if rank == 0:
         achieved = flops_attn / (attn_ms * 1e-3) / 1e12

@@ -206,6 +206,27 @@ chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk,
 chorus_status chorus_mask_coverage(const float* mass, const uint32_t* bitmask, int heads, int nq_blk,
                                    int nk_blk, float* coverage, void* cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Head-level scheduling for load balance (PAPER.md:L95 and appendix A): with a reused
+ * mask the cost of every head is known before the attention runs, so heads are re-partitioned over
+ * the ranks of a sequence-parallel (Ulysses) group before the all-to-all.
+ *
+ * chorus_head_costs: cost[h] = kept tiles of head h = row_ptr[(h+1)*nq_blk] - row_ptr[h*nq_blk].
+ *   row_ptr  device, int32, this layer's H*nq_blk + 1 entries;  cost  device, int64 [H].
+ * chorus_schedule_heads (HOST function, no device work): heads in order of decreasing cost (ties:
+ *   lower head first) go to the rank with the lightest current load among the ranks that still have
+ *   room (ties: lower rank); a rank takes at most cap = ceil(H / n_ranks) heads (R24).
+ *   cost     host, int64 [H], >= 0.
+ *   order    host, int32 [n_ranks * cap]: order[r*cap + i] = i-th head of rank r (ascending inside a
+ *            rank), -1 in unused slots.  n_ranks == 1 gives 0, 1, ..., H-1 (a no-op, Table 4).
+ *   load     host, int64 [n_ranks] or NULL: summed cost per rank.
+ * Errors: INVALID_ARG (null, H/n_ranks/nq_blk <= 0, negative cost), CUDA (head_costs only).
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_head_costs(const int32_t* row_ptr, int H, int nq_blk, int64_t* cost,
+                                void* cuda_stream);
+chorus_status chorus_schedule_heads(const int64_t* cost, int H, int n_ranks, int32_t* order,
+                                    int64_t* load);
+
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char* chorus_last_error(void);
 

@@ -191,3 +191,24 @@ def mask_coverage(mass, bitmask, nk):
     out = np.zeros(heads, dtype=np.float64)
     lib().oracle_mask_coverage(_p(m), _p(b), heads, nq, nk, _p(out))
     return out
+
+
+def schedule_heads(cost, n_ranks):
+    """Head-level scheduling (appendix A), followed step by step: heads with
+    the heavier workload first, each "to the GPUs with the lightest current load"; a rank takes at
+    most ceil(H / n_ranks) heads (equal head slots per rank under Ulysses, R24); ties:
+    lower head, lower rank.  Returns (list of ascending head lists per rank, loads)."""
+    cost = [int(c) for c in cost]
+    H = len(cost)
+    cap = -(-H // n_ranks)
+    heads = sorted(range(H), key=lambda h: (-cost[h], h))
+    mine = [[] for _ in range(n_ranks)]
+    load = [0] * n_ranks
+    for h in heads:
+        best = None
+        for r in range(n_ranks):
+            if len(mine[r]) < cap and (best is None or load[r] < load[best]):
+                best = r
+        mine[best].append(h)
+        load[best] += cost[h]
+    return [sorted(m) for m in mine], load

@@ -20,7 +20,7 @@ BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
 
 EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
-           "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_last_error", "chorus_version",
+           "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count"]
 
 
@@ -72,6 +72,8 @@ def lib() -> C.CDLL:
                                             C.c_void_p, C.c_void_p, C.c_void_p]
         L.chorus_mask_coverage.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
                                            C.c_void_p, C.c_void_p]
+        L.chorus_head_costs.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.chorus_schedule_heads.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -254,3 +256,23 @@ def chorus_mask_coverage(mass, bitmask, nk_blk: int, coverage=None, stream=None)
     _check(lib().chorus_mask_coverage(_ptr(mass), _ptr(bitmask), heads, nq, nk, _ptr(coverage),
                                       _stream(stream)))
     return coverage
+
+
+def chorus_head_costs(row_ptr, H: int, nq_blk: int, cost=None, stream=None):
+    """Kept tiles per head from this layer's CSR row_ptr (cuda int32) -> int64 [H] (cuda)."""
+    if cost is None:
+        cost = torch.empty(H, dtype=torch.int64, device=row_ptr.device)
+    _check(lib().chorus_head_costs(_ptr(row_ptr), H, nq_blk, _ptr(cost), _stream(stream)))
+    return cost
+
+
+def chorus_schedule_heads(cost, n_ranks: int):
+    """Host call (appendix A): cost = int64 [H] (host tensor or sequence).  Returns
+    (order int32 [n_ranks][cap], load int64 [n_ranks]); -1 marks unused slots."""
+    cost = torch.as_tensor(cost, dtype=torch.int64).contiguous().cpu()
+    H = cost.numel()
+    cap = (H + n_ranks - 1) // n_ranks
+    order = torch.empty((n_ranks, cap), dtype=torch.int32)
+    load = torch.empty(n_ranks, dtype=torch.int64)
+    _check(lib().chorus_schedule_heads(_ptr(cost), H, n_ranks, _ptr(order), _ptr(load)))
+    return order, load

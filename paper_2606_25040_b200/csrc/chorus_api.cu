@@ -260,6 +260,26 @@ chorus_status chorus_mask_coverage(const float* mass, const uint32_t* bitmask, i
                                            static_cast<cudaStream_t>(cuda_stream)), "mask_coverage launch");
 }
 
+chorus_status chorus_head_costs(const int32_t* row_ptr, int H, int nq_blk, int64_t* cost,
+                                void* cuda_stream) {
+    g_err[0] = 0;
+    if (!row_ptr || !cost) return set_error(CHORUS_ERR_INVALID_ARG, "row_ptr / cost is null");
+    if (H <= 0 || nq_blk <= 0) return set_error(CHORUS_ERR_INVALID_ARG, "H, nq_blk must be positive");
+    return check_cuda(launch_head_costs(row_ptr, H, nq_blk, cost, static_cast<cudaStream_t>(cuda_stream)),
+                      "head_costs launch");
+}
+
+chorus_status chorus_schedule_heads(const int64_t* cost, int H, int n_ranks, int32_t* order,
+                                    int64_t* load) {
+    g_err[0] = 0;
+    if (!cost || !order) return set_error(CHORUS_ERR_INVALID_ARG, "cost / order is null");
+    if (H <= 0 || n_ranks <= 0) return set_error(CHORUS_ERR_INVALID_ARG, "H, n_ranks must be positive");
+    for (int h = 0; h < H; ++h)
+        if (cost[h] < 0) return set_error(CHORUS_ERR_INVALID_ARG, "cost[%d] is negative", h);
+    schedule_heads_host(cost, H, n_ranks, order, load);
+    return CHORUS_OK;
+}
+
 chorus_status chorus_quantize_fp8(const void* Q, const void* K, const void* V,
                                   const chorus_attn_shape* shape, void* q8, void* k8, void* v8,
                                   float* q_scale, float* k_scale, float* v_scale,

@@ -57,4 +57,8 @@ cudaError_t launch_mask_from_mass(const float* mass, int64_t rows, int nk, doubl
 cudaError_t launch_mask_coverage(const float* mass, const uint32_t* bitmask, int heads, int nq, int nk,
                                  float* coverage, cudaStream_t stream);
 
+// ---- head_schedule.cu --------------------------------------------------------------------------
+cudaError_t launch_head_costs(const int32_t* row_ptr, int H, int nq, int64_t* cost, cudaStream_t stream);
+void schedule_heads_host(const int64_t* cost, int H, int n_ranks, int32_t* order, int64_t* load);
+
 }  // namespace chorus

@@ -79,3 +79,19 @@ def test_visit_refresh_matches_oracle():
     B.chorus_visit_refresh(d, nk, group=8)
     torch.cuda.synchronize()
     assert np.array_equal(d.cpu().numpy().view(np.uint32), ref)
+
+
+def test_head_costs_from_row_ptr():
+    # PAPER.md:L95 / appendix A: the per-head cost is known from the reused mask before attention runs
+    cfg = W.scaled(W.CFG2, H=6)
+    bm = np.stack([W.layer_mask(cfg, seed=5, density=0.05 + 0.1 * 0)] )[0]
+    for h in range(cfg.H):                           # different density per head
+        bm[h] = W.layer_mask(W.scaled(cfg, H=1), seed=40 + h, density=0.05 + 0.07 * h)[0]
+    rp, _ = B.chorus_mask_to_index(dmask(bm[None]), cfg.nk)
+    cost = B.chorus_head_costs(rp, cfg.H, cfg.nq)
+    torch.cuda.synchronize()
+    want = W.unpack_bits(bm, cfg.nk).reshape(cfg.H, -1).sum(axis=1)
+    assert np.array_equal(cost.cpu().numpy(), want)
+    order, load = B.chorus_schedule_heads(cost.cpu(), 3)
+    mine, load_o = oracle.schedule_heads(want, 3)
+    assert [[h for h in r.tolist() if h >= 0] for r in order] == mine and load.tolist() == load_o

@@ -1,0 +1,42 @@
+"""The N > 1 path of bench.py on CPU: world_size 2 over gloo.  The hot path itself does not shard
+("replicas only"), so what N > 1 adds is the reduction of the per-rank device
+times (max over ranks) and the whole-job aggregate; both are exercised here with two processes."""
+import os
+
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+import bench
+
+
+def _worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    times = [10.0 + rank, 30.0 - 5 * rank]            # rank 1 is slower on the first, rank 0 on the second
+    red = bench.max_over_ranks(times, torch.device("cpu"), world)
+    dist.barrier()
+    if rank == 0:
+        out.put(red)
+    dist.destroy_process_group()
+
+
+def test_max_over_ranks_two_processes():
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = 31500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    red = out.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert red == [11.0, 30.0]
+
+
+def test_single_rank_is_identity_and_aggregate_scales_with_replicas():
+    assert bench.max_over_ranks([1.5, 2.5], torch.device("cpu"), 1) == [1.5, 2.5]
+    one = bench.whole_job_value(1, 5.5e12, 4.4)
+    assert abs(one - 1250.0) < 1e-9
+    assert bench.whole_job_value(8, 5.5e12, 4.4) == 8 * one      # weak scaling: same time, 8x the work
