@@ -326,6 +326,39 @@ def run_chorus(args):
     e2e_ms = a.elapsed_time(b_) / e2e_steps
     clocks = sampler.stop() if rank == 0 else None
 
+    # optional: the density sweep of BASELINE.json configs[4] (5/10/25/50/100 % on one layer; 100 % is
+    # dense attention through the same kernel), outside the timed region, rank 0 only
+    sweep = None
+    if rank == 0 and args.sweep:
+        sweep = []
+        for rho in (0.05, 0.10, 0.25, 0.50, 1.0):
+            bms = W.layer_mask(cfg, density=rho)
+            dMs_ = torch.from_numpy(bms[None].view(np.int32)).to(dev)
+            rho_real = W.mask_density(bms, cfg.nk)
+            rp_, ci_ = B.chorus_mask_to_index(dMs_, cfg.nk)
+            ent = {"density": rho_real, "flops": attn_flops(cfg, rho_real)}
+            for name, fn in (("bf16", lambda: B.chorus_block_sparse_attn_fwd(dQ, dK, dV, rp_, ci_, cfg.scale, O=dO)),
+                             ("fp8", (lambda: B.chorus_block_sparse_attn_fwd(q8[0], q8[1], q8[2], rp_, ci_, cfg.scale,
+                                                                             dtype=B.CHORUS_FP8_E4M3, O=dO8, fp8_scales=q8[3:]))
+                              if has_fp8 else None)):
+                if fn is None:
+                    continue
+                for _ in range(3):
+                    fn()
+                torch.cuda.synchronize()
+                ts = []
+                for _ in range(7):
+                    a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream); fn(); b_.record(stream)
+                    torch.cuda.synchronize()
+                    ts.append(a.elapsed_time(b_))
+                ms = statistics.median(ts)
+                tf = ent["flops"] / (ms * 1e-3) / 1e12
+                ent[name] = {"ms": ms, "TFLOPs": tf,
+                             "frac_of_peak": tf / (peaks["bf16"] * (2 if name == "fp8" else 1))}
+            sweep.append(ent)
+            del dMs_, rp_, ci_
+
     # mask decode at the size where it is HBM-bound: a whole stored mask set (40 layers x H heads,
     # SURVEY section 8 d-4), timed alone with a flushed L2; reported beside the per-layer figure
     set_ms = set_bytes = None
@@ -394,6 +427,8 @@ def run_chorus(args):
                                       "decode_set_GBps": set_bytes / (set_ms * 1e-3) / 1e9,
                                       "decode_set_frac_of_hbm": set_bytes / (set_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                                       "decode_set": "40 layers x %d heads x %d rows, L2 flushed, median of 5" % (cfg.H, cfg.nq)})
+        if sweep is not None:
+            line["density_sweep"] = sweep
         if has_fp8:
             a8 = flops_attn / (attn8_ms * 1e-3) / 1e12
             line["breakdown"].update({"quantize_ms": quant_ms, "attn_fp8_ms": attn8_ms, "attn_fp8_TFLOPs": a8,
@@ -420,6 +455,8 @@ def main():
     ap.add_argument("--no-fp8", dest="fp8", action="store_false", default=True,
                     help="leave the FP8 leg (quantise + FP8 attention) out of the step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="add the 5/10/25/50/100 %% density sweep of one layer to the JSON line (off by default)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "chorus" else args.warmup
     if args.impl == "reference":
