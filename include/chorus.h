@@ -135,6 +135,19 @@ chorus_status chorus_block_sparse_attn_fwd(const void* Q, const void* K, const v
                                            const chorus_attn_shape* shape,
                                            const chorus_fp8_scales* fp8, void* cuda_stream);
 
+/* The same call with one more output: lse[b][h][i] = log sum_{j in J(i)} exp(scale * <Q[i], K[j]>)
+ * (natural log, fp32, PACKED [B][H][N]; -inf for a row with no kept block).  With a full mask this
+ * is the row statistic of the dense attention that chorus_block_mass can reuse (the
+ * historical request records its mask "as a by-product" of its own attention).  For FP8 inputs the
+ * scores are those of the dequantised Q and K.  lse == NULL behaves like the call above.
+ * Accuracy against the fp64 oracle: |err| <= 2e-3 (bf16), 2e-2 (fp8). */
+chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, const void* V,
+                                               const int32_t* row_ptr, const int32_t* col_idx,
+                                               float scale, chorus_dtype dtype, void* O,
+                                               const chorus_attn_shape* shape,
+                                               const chorus_fp8_scales* fp8, float* lse,
+                                               void* cuda_stream);
+
 /* ---------------------------------------------------------------------------------------------
  * FP8 quantisation pre-pass for dtype = CHORUS_FP8_E4M3 (PAPER.md:L97 says only "FP8
  * quantization"; granularity and formula are BASELINE.json configs[2] / DESIGN.md R10-R11):
@@ -178,6 +191,9 @@ chorus_status chorus_retrieve_top1(const float* bank, int n, int dim, const floa
  *   attention).  Every valid query row contributes exactly 1.
  *   Q, K     device, bf16, [B][N][H][d] with the q_/k_ strides of `shape` (v_/o_ strides ignored);
  *            16-byte aligned, strides multiples of 8 elements, d = 128.
+ *   lse      device, float [B][H][N] or NULL: the rows' log-sum-exp (natural log) of the SAME dense
+ *            attention, as written by chorus_block_sparse_attn_fwd_lse with a full mask.  Given, the
+ *            kernel makes one pass over the keys instead of two (half the MMAs and exponentials).
  *   mass     device, float [B][H][ceil(N/128)][ceil(N/64)], fully overwritten.
  *   Accuracy against the fp64 oracle: |err| <= 2e-3 * max(mass, 1e-3) + 1e-5 per block (bf16
  *   products, fp32 sums, ex2.approx); the result is deterministic (fixed summation order).
@@ -199,7 +215,8 @@ chorus_status chorus_retrieve_top1(const float* bank, int n, int dim, const floa
  *         UNSUPPORTED (d != 128, nk_blk > 2048), CUDA.
  * ------------------------------------------------------------------------------------------- */
 chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
-                                const chorus_attn_shape* shape, float* mass, void* cuda_stream);
+                                const chorus_attn_shape* shape, const float* lse, float* mass,
+                                void* cuda_stream);
 chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk, float top_p,
                                     float min_top_k, uint32_t* bitmask, int32_t* kept,
                                     void* cuda_stream);

@@ -69,13 +69,14 @@ def _strides(a):
 
 
 def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_threads=0,
-                      return_weight_sum=False):
+                      return_weight_sum=False, return_lse=False):
     """fp64 block-sparse attention on the exact input bytes.
 
     Q, K, V: [B][N][H][d] numpy arrays, uint16 (bf16 bits) or uint8 (e4m3 codes; then
     fp8_scales = (q_scale [B][H][ceil(N/128)], k_scale same, v_scale [B][H][d]) float32).
     bitmask: uint32 [H][nq][words] (one layer).  items: int array [n][3] of (b, h, qb); default all.
-    Returns out float64 [n_items][128][d] (rows beyond N are 0)  (+ weight sums [n_items][128]).
+    Returns out float64 [n_items][128][d] (rows beyond N are 0)  (+ weight sums [n_items][128])
+    (+ row log-sum-exp [n_items][128], natural log, -inf for empty rows, if return_lse).
     """
     assert Q.dtype == K.dtype == V.dtype and Q.dtype in (np.uint16, np.uint8)
     dtype = 0 if Q.dtype == np.uint16 else 1
@@ -91,6 +92,7 @@ def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_th
     n = items.shape[0]
     out = np.zeros((n, BQ, d), dtype=np.float64)
     ws = np.zeros((n, BQ), dtype=np.float64) if return_weight_sum else None
+    lse = np.zeros((n, BQ), dtype=np.float64) if return_lse else None
     if dtype:
         qs, ks, vs = (_c(x, np.float32) for x in fp8_scales)
         nsb = (N + 127) // 128
@@ -101,8 +103,9 @@ def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_th
         _p(Q), _p(K), _p(V), C.c_int(dtype), B, H, N, d,
         *_strides(Q), *_strides(K), *_strides(V),
         _p(qs), _p(ks), _p(vs), _p(bm), C.c_double(scale),
-        n, _p(ib), _p(ih), _p(iq), _p(out), _p(ws), C.c_int(n_threads))
-    return (out, ws) if return_weight_sum else out
+        n, _p(ib), _p(ih), _p(iq), _p(out), _p(ws), _p(lse), C.c_int(n_threads))
+    res = (out,) + ((ws,) if return_weight_sum else ()) + ((lse,) if return_lse else ())
+    return res if len(res) > 1 else out
 
 
 def scatter_items(out_items, items, N, H):

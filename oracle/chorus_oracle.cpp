@@ -146,6 +146,8 @@ int64_t oracle_mask_to_index(const uint32_t* bitmask, int L, int H, int nq, int 
 // out[t][r][c] (r < 128, c < d) as doubles; rows with 128*qb + r >= N are written as 0.
 // bitmask is one layer: [H][nq][words].  Strides are in elements; the last dim is contiguous.
 // If weight_sum != null, weight_sum[t][r] receives sum_j p_j / l (must be 1; 0 for an empty row).
+// If lse != null, lse[t][r] receives the row's log-sum-exp m + log(l) = log sum_{j in J} exp(s_j)
+// (natural log; -inf for an empty row or a row >= N).
 // -------------------------------------------------------------------------------------------------
 void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int dtype,
                               int B, int H, int N, int d,
@@ -156,7 +158,7 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
                               const uint32_t* bitmask, double scale,
                               int n_items, const int32_t* item_b, const int32_t* item_h,
                               const int32_t* item_qb, double* out, double* weight_sum,
-                              int n_threads) {
+                              double* lse, int n_threads) {
     (void)B;
     const int nq = (N + BQ - 1) / BQ;
     const int nk = (N + BK - 1) / BK;
@@ -206,6 +208,7 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
                 const int i = qb * BQ + r;
                 for (int c = 0; c < d; ++c) o[c] = 0.0;
                 if (weight_sum) weight_sum[static_cast<int64_t>(t) * BQ + r] = 0.0;
+                if (lse) lse[static_cast<int64_t>(t) * BQ + r] = -std::numeric_limits<double>::infinity();
                 if (i >= N || nj == 0) continue;
 
                 const double qs = dtype ? static_cast<double>(
@@ -227,6 +230,7 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
                     for (int c = 0; c < d; ++c) acc[c] += p * Vd[x * d + c];
                 }
                 for (int c = 0; c < d; ++c) o[c] = acc[c] / l;
+                if (lse) lse[static_cast<int64_t>(t) * BQ + r] = m + std::log(l);
                 if (weight_sum) {
                     double w = 0.0;
                     for (size_t x = 0; x < nj; ++x) w += std::exp(s[x] - m) / l;

@@ -19,6 +19,7 @@ CHORUS_BF16, CHORUS_FP8_E4M3 = 0, 1
 BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
 
 EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
+           "chorus_block_sparse_attn_fwd_lse",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
            "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count"]
@@ -67,7 +68,11 @@ def lib() -> C.CDLL:
                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.POINTER(C.c_size_t), C.c_void_p]
         L.chorus_block_mass.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.POINTER(AttnShape),
-                                        C.c_void_p, C.c_void_p]
+                                        C.c_void_p, C.c_void_p, C.c_void_p]
+        L.chorus_block_sparse_attn_fwd_lse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                                       C.c_void_p, C.c_float, C.c_int, C.c_void_p,
+                                                       C.POINTER(AttnShape), C.POINTER(Fp8Scales),
+                                                       C.c_void_p, C.c_void_p]
         L.chorus_mask_from_mass.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_float, C.c_float,
                                             C.c_void_p, C.c_void_p, C.c_void_p]
         L.chorus_mask_coverage.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
@@ -160,7 +165,7 @@ def attn_shape(Q, K, V, O=None) -> AttnShape:
 
 
 def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype: int = CHORUS_BF16,
-                                 O=None, fp8_scales=None, stream=None):
+                                 O=None, fp8_scales=None, stream=None, lse=None):
     """Q, K, V: cuda tensors indexed [B][N][H][d] (bf16, or uint8/float8_e4m3fn codes for FP8).
     row_ptr: this layer's H*nq+1 entries (a view into the full row_ptr is fine).  Returns O (bf16)."""
     assert Q.is_cuda and K.is_cuda and V.is_cuda
@@ -171,6 +176,13 @@ def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype:
     sc = None
     if fp8_scales is not None:
         sc = Fp8Scales(*(x.data_ptr() for x in fp8_scales))
+    if lse is not None:     # float32 [B][H][N], written by the kernel (natural-log row log-sum-exp)
+        assert lse.dtype == torch.float32 and lse.is_contiguous() and lse.shape == (B, H, N)
+        _check(lib().chorus_block_sparse_attn_fwd_lse(_ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx),
+                                                      C.c_float(scale), dtype, _ptr(O), C.byref(shape),
+                                                      C.byref(sc) if sc is not None else None,
+                                                      _ptr(lse), _stream(stream)))
+        return O
     _check(lib().chorus_block_sparse_attn_fwd(_ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx),
                                               C.c_float(scale), dtype, _ptr(O), C.byref(shape),
                                               C.byref(sc) if sc is not None else None,
@@ -219,7 +231,7 @@ def chorus_retrieve_top1(bank, query, tau: float, out=None, workspace=None, stre
     return out
 
 
-def chorus_block_mass(Q, K, scale: float, mass=None, stream=None):
+def chorus_block_mass(Q, K, scale: float, mass=None, stream=None, lse=None):
     """bf16 Q, K [B][N][H][d] (cuda) -> float32 mass [B][H][ceil(N/128)][ceil(N/64)] of the dense
     attention (PAPER.md:L73, L81)."""
     B, N, H, d = Q.shape
@@ -227,8 +239,8 @@ def chorus_block_mass(Q, K, scale: float, mass=None, stream=None):
     if mass is None:
         mass = torch.empty((B, H, nq, nk), dtype=torch.float32, device=Q.device)
     shape = attn_shape(Q, K, K)
-    _check(lib().chorus_block_mass(_ptr(Q), _ptr(K), C.c_float(scale), C.byref(shape), _ptr(mass),
-                                   _stream(stream)))
+    _check(lib().chorus_block_mass(_ptr(Q), _ptr(K), C.c_float(scale), C.byref(shape), _ptr(lse),
+                                   _ptr(mass), _stream(stream)))
     return mass
 
 

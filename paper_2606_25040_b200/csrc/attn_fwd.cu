@@ -582,6 +582,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const float a_oth = (m_oth == -INFINITY) ? 0.f : ex2(m_oth - m_all);
             const float L = l_mine * a_mine + l_oth * a_oth;
             const float inv = (L > 0.f) ? 1.f / L : 0.f;
+            // optional row log-sum-exp (natural log of sum_j exp(scale * q . k_j) over the retained
+            // keys; -inf for an empty row): what a later block-mass pass needs
+            if (p.lse != nullptr && sm == 0 && it.qb * BQ + row < p.N)
+                p.lse[(static_cast<int64_t>(it.b) * p.H + it.h) * p.N + it.qb * BQ + row] =
+                    (L > 0.f) ? (m_all + lg2(L) - C::P_SHIFT) * 0.6931471805599453f : -INFINITY;
             named_bar_sync(NB_HALF + sm, 128);                 // staging free for the whole warpgroup
             if (it.nt > 0) {
                 mbar_wait(bar(C::B_ITEM_DONE), icnt & 1);      // every P V of the item has completed

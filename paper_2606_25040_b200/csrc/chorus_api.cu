@@ -170,6 +170,16 @@ chorus_status chorus_block_sparse_attn_fwd(const void* Q, const void* K, const v
                                            float scale, chorus_dtype dtype, void* O,
                                            const chorus_attn_shape* shape,
                                            const chorus_fp8_scales* fp8, void* cuda_stream) {
+    return chorus_block_sparse_attn_fwd_lse(Q, K, V, row_ptr, col_idx, scale, dtype, O, shape, fp8,
+                                            nullptr, cuda_stream);
+}
+
+chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, const void* V,
+                                               const int32_t* row_ptr, const int32_t* col_idx,
+                                               float scale, chorus_dtype dtype, void* O,
+                                               const chorus_attn_shape* shape,
+                                               const chorus_fp8_scales* fp8, float* lse,
+                                               void* cuda_stream) {
     g_err[0] = 0;
     if (dtype != CHORUS_BF16 && dtype != CHORUS_FP8_E4M3)
         return set_error(CHORUS_ERR_UNSUPPORTED, "unknown dtype %d", static_cast<int>(dtype));
@@ -209,6 +219,7 @@ chorus_status chorus_block_sparse_attn_fwd(const void* Q, const void* K, const v
     p.q_scale = fp8 ? fp8->q_scale : nullptr;
     p.k_scale = fp8 ? fp8->k_scale : nullptr;
     p.v_scale = fp8 ? fp8->v_scale : nullptr;
+    p.lse = lse;
     cudaError_t e = launch_attn_fwd(tmQ, tmK, tmV, tmO, p, dtype, static_cast<cudaStream_t>(cuda_stream));
     if (e == cudaErrorNotSupported)
         return set_error(CHORUS_ERR_UNSUPPORTED, "dtype %d not implemented by this build", (int)dtype);
@@ -216,7 +227,8 @@ chorus_status chorus_block_sparse_attn_fwd(const void* Q, const void* K, const v
 }
 
 chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
-                                const chorus_attn_shape* shape, float* mass, void* cuda_stream) {
+                                const chorus_attn_shape* shape, const float* lse, float* mass,
+                                void* cuda_stream) {
     g_err[0] = 0;
     if (!Q || !K || !mass) return set_error(CHORUS_ERR_INVALID_ARG, "Q, K, mass must be non-null");
     if (!aligned16(Q) || !aligned16(K)) return set_error(CHORUS_ERR_INVALID_ARG, "Q, K must be 16-byte aligned");
@@ -231,7 +243,7 @@ chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
                         64, 128, "Q")) != CHORUS_OK) return st;
     if ((st = make_tmap(&tmK, K, 2, s.B, s.H, s.N, s.d, s.k_stride_b, s.k_stride_n, s.k_stride_h,
                         64, 128, "K")) != CHORUS_OK) return st;
-    return check_cuda(launch_block_mass(tmQ, tmK, mass, s.B, s.H, s.N, scale * 1.4426950408889634f,
+    return check_cuda(launch_block_mass(tmQ, tmK, lse, mass, s.B, s.H, s.N, scale * 1.4426950408889634f,
                                         static_cast<cudaStream_t>(cuda_stream)), "block mass launch");
 }
 

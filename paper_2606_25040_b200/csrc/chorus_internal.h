@@ -44,14 +44,15 @@ struct AttnParams {
     const float* q_scale;
     const float* k_scale;
     const float* v_scale;
+    float* lse;  // optional [B][H][N] row log-sum-exp (natural log), or null
 };
 cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
                             cudaStream_t stream);
 
 // ---- mask_build.cu -----------------------------------------------------------------------------
-cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, float* mass, int B, int H,
-                              int N, float scale_log2, cudaStream_t stream);
+cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, const float* lse, float* mass,
+                              int B, int H, int N, float scale_log2, cudaStream_t stream);
 cudaError_t launch_mask_from_mass(const float* mass, int64_t rows, int nk, double top_p, double min_top_k,
                                   uint32_t* bitmask, int32_t* kept, cudaStream_t stream);
 cudaError_t launch_mask_coverage(const float* mass, const uint32_t* bitmask, int heads, int nq, int nk,

@@ -24,6 +24,8 @@ using namespace ptx;
 // over its P pairs: steps 0..P-1 give every row its running maximum and sum (-> log-sum-exp), steps
 // P..2P-1 recompute the same scores and sum exp2(s - lse) over the rows and the 64 columns of each
 // block.  Recomputing QK^T costs a second MMA pass, but nothing of size N x N is ever stored.
+// When the caller hands in the rows' log-sum-exp (an output of the dense attention call that the
+// historical request makes anyway), the first pass is skipped (template kLse).
 //   warp 8      TMA producer: Q once per item, then the K pair of every step (ring of KST stages)
 //   warp 9      MMA issuer: S = Q K^T (M=128, N=128, K=128, bf16 -> fp32) into one of four S buffers
 //               in tensor memory, up to four steps ahead of the readers
@@ -41,10 +43,12 @@ static_assert(B_CNT * 8 + 8 <= 256, "barrier area too small");
 
 struct MassParams {
     float* mass;
+    const float* lse;   // optional [B][H][N] natural-log row log-sum-exp of the SAME dense attention
     int B, H, N, nq, nk;
     float scale_log2;
 };
 
+template <bool kLse>   // the rows' log-sum-exp is given: one pass over the keys instead of two
 __global__ void __launch_bounds__(MB_THREADS, 1)
 block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const MassParams p) {
@@ -60,6 +64,9 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_items = p.B * p.H * p.nq;
     const int P = (p.nk + 1) >> 1;       // pairs per item
+    // With the rows' log-sum-exp given (an output of the dense attention call) the first pass is
+    // skipped: P steps instead of 2 P, one exponential per score instead of two.
+    const int T = kLse ? P : 2 * P;       // steps per item
     if (threadIdx.x == 0) {
         mbar_init(bar(B_Q_FULL), 1);
         mbar_init(bar(B_Q_EMPTY), 1);
@@ -85,7 +92,7 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                 tma_load_4d(sQ + 16384, &tmQ, bar(B_Q_FULL), 64, qb * 128, h, b);
             }
             __syncwarp();
-            for (int t = 0; t < 2 * P; ++t) {
+            for (int t = 0; t < T; ++t) {
                 const int j = t < P ? t : t - P;
                 mbar_wait(bar(B_K_EMPTY + st), ph ^ 1);
                 if (elect_one()) {
@@ -105,7 +112,7 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         uint32_t st = 0, ph = 0, icnt = 0, g = 0;
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x, ++icnt) {
             mbar_wait(bar(B_Q_FULL), icnt & 1);
-            for (int t = 0; t < 2 * P; ++t, ++g) {
+            for (int t = 0; t < T; ++t, ++g) {
                 const uint32_t sb = g % SB;
                 mbar_wait(bar(B_K_FULL + st), ph);
                 if (g >= SB) mbar_wait(bar(B_S_FREE + sb), ((g - SB) / SB) & 1);
@@ -120,7 +127,7 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     }
                     tc_commit(bar(B_K_EMPTY + st));
                     tc_commit(bar(B_S_FULL + sb));
-                    if (t == 2 * P - 1) tc_commit(bar(B_Q_EMPTY));
+                    if (t == T - 1) tc_commit(bar(B_Q_EMPTY));
                 }
                 __syncwarp();
                 if (++st == KST) { st = 0; ph ^= 1; }
@@ -135,9 +142,11 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             const int qb = idx % p.nq;
             const bool row_ok = qb * 128 + row < p.N;
             float m = -INFINITY, l = 0.f, lse2 = 0.f;
+            if (kLse && row_ok)                 // natural log -> the log2 domain of the scores
+                lse2 = __ldg(p.lse + static_cast<int64_t>(idx / p.nq) * p.N + qb * 128 + row) * 1.4426950408889634f;
             uint32_t own = 0;                   // this group's steps of the item so far (xpart buffer)
-            for (int t = 0; t < 2 * P; ++t) {
-                if (t == P) {
+            for (int t = 0; t < T; ++t) {
+                if (!kLse && t == P) {
                     // ---- pass boundary: combine the two groups' (m, l) into the row's log-sum-exp
                     xst[(grp * 2 + 0) * 128 + row] = m;
                     xst[(grp * 2 + 1) * 128 + row] = l;
@@ -168,7 +177,7 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                         if (lane == 0) mbar_arrive(bar(B_S_FREE + sb));
                     }
                     const int vc = valid - 32 * c;           // valid columns of this chunk
-                    if (t < P) {
+                    if (!kLse && t < P) {
                         float cm = -INFINITY;
 #pragma unroll
                         for (int k = 0; k < 32; ++k)
@@ -191,7 +200,7 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                         if (c < 2) sum_a += acc; else sum_b += acc;
                     }
                 }
-                if (t >= P) {
+                if (kLse || t >= P) {
                     // ---- sums over the 128 rows: lanes, then the four warps in a fixed order ------
                     if (!row_ok) { sum_a = 0.f; sum_b = 0.f; }
 #pragma unroll
@@ -212,7 +221,7 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     ++own;
                 }
             }
-            g0 += 2 * P;
+            g0 += T;
         }
     }
     tc_fence_before();
@@ -346,21 +355,25 @@ mask_coverage_kernel(const float* __restrict__ mass, const uint32_t* __restrict_
 
 }  // namespace
 
-cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, float* mass, int B, int H,
-                              int N, float scale_log2, cudaStream_t stream) {
-    cudaError_t e = cudaFuncSetAttribute(block_mass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, M_SMEM);
+cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, const float* lse, float* mass,
+                              int B, int H, int N, float scale_log2, cudaStream_t stream) {
+    cudaError_t e = lse ? cudaFuncSetAttribute(block_mass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, M_SMEM)
+                        : cudaFuncSetAttribute(block_mass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, M_SMEM);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     MassParams p;
     p.mass = mass;
+    p.lse = lse;
     p.B = B; p.H = H; p.N = N;
     p.nq = (N + 127) / 128;
     p.nk = (N + 63) / 64;
     p.scale_log2 = scale_log2;
     const int n_items = B * H * p.nq;
-    block_mass_kernel<<<n_items < sms ? n_items : sms, MB_THREADS, M_SMEM, stream>>>(tmQ, tmK, p);
+    const int grid = n_items < sms ? n_items : sms;
+    if (lse) block_mass_kernel<true><<<grid, MB_THREADS, M_SMEM, stream>>>(tmQ, tmK, p);
+    else block_mass_kernel<false><<<grid, MB_THREADS, M_SMEM, stream>>>(tmQ, tmK, p);
     count_launch(1);
     return cudaGetLastError();
 }

@@ -150,3 +150,25 @@ def test_cfg4_720p_stress_rows_sampled_blocks():
     bm = W.layer_mask(cfg)
     items = sample_items(cfg.H, cfg.nq, 5, seed=1, always=[(0, 3, cfg.nq - 1)])
     compare(cfg, Q, K, V, bm, items, stress=True)
+
+
+def test_fp8_lse_output():
+    # scores of the dequantised Q and K; the 2^5 shift of P must not leak into the log-sum-exp
+    import oracle
+    cfg = W.scaled(W.CFG1, H=2)
+    Q, K, V = W.qkv_bits(cfg)
+    bm = W.layer_mask(cfg)
+    from gpu_common import dbf16, dev
+    rp, ci = B.chorus_mask_to_index(torch.from_numpy(bm[None].view(np.int32)).to(dev()), cfg.nk)
+    q8 = B.chorus_quantize_fp8(dbf16(Q), dbf16(K), dbf16(V))
+    lse = torch.zeros((1, cfg.H, cfg.N), dtype=torch.float32, device=dev())
+    B.chorus_block_sparse_attn_fwd(q8[0], q8[1], q8[2], rp, ci, cfg.scale, dtype=B.CHORUS_FP8_E4M3,
+                                   fp8_scales=q8[3:], lse=lse)
+    torch.cuda.synchronize()
+    items = np.array([(0, 0, 0), (0, 1, 5), (0, 1, cfg.nq - 1)], np.int32)
+    codes = [x.cpu().numpy() for x in q8[:3]]
+    scales = [x.cpu().numpy() for x in q8[3:]]
+    _, lse_o = oracle.block_sparse_attn(*codes, bm, cfg.scale, items=items, fp8_scales=scales, return_lse=True)
+    got = lse.cpu().numpy().astype(np.float64)
+    for t, (_, h, qb) in enumerate(items):
+        assert np.abs(got[0, h, 128 * qb: 128 * qb + 128] - lse_o[t]).max() <= 2e-2

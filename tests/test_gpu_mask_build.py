@@ -118,3 +118,50 @@ def test_true_top_p_mask_of_one_full_size_head():
     rp, ci = B.chorus_mask_to_index(bm[None], cfg.nk)
     rp_o, ci_o = oracle.mask_to_index(bm_o[None], cfg.nk)
     assert np.array_equal(rp.cpu().numpy(), rp_o) and np.array_equal(ci.cpu().numpy()[: len(ci_o)], ci_o)
+
+
+def test_attention_lse_output_and_single_pass_mass():
+    # the mask is a by-product of the historical request's own (dense) attention: its
+    # row log-sum-exp feeds the block-mass pass, which then needs one sweep over the keys, not two
+    N, H, scale = 1000, 2, 0.2
+    Q, K, V = random_qkv_bits(N, H, seed=31)
+    nq, nk = (N + 127) // 128, (N + 63) // 64
+    full = W.pack_bits(np.ones((H, nq, nk), dtype=bool))
+    tq, tk, tv = dbf16(Q), dbf16(K), dbf16(V)
+    rp, ci = B.chorus_mask_to_index(torch.from_numpy(full[None].view(np.int32)).to(dev()), nk)
+    lse = torch.full((1, H, N), 7.0, dtype=torch.float32, device=dev())
+    O = B.chorus_block_sparse_attn_fwd(tq, tk, tv, rp, ci, scale, lse=lse)
+    O_plain = B.chorus_block_sparse_attn_fwd(tq, tk, tv, rp, ci, scale)
+    torch.cuda.synchronize()
+    assert torch.equal(O, O_plain)                                        # the extra output changes nothing
+    items = np.array([(0, h, qb) for h in range(H) for qb in range(nq)], np.int32)
+    _, lse_o = oracle.block_sparse_attn(Q, K, V, full, scale, items=items, return_lse=True)
+    got = lse.cpu().numpy().astype(np.float64)
+    for t, (_, h, qb) in enumerate(items):
+        n = min(128, N - 128 * qb)
+        assert np.abs(got[0, h, 128 * qb: 128 * qb + n] - lse_o[t, :n]).max() <= 2e-3
+    ref = oracle.block_mass(Q, K, scale)
+    two_pass = B.chorus_block_mass(tq, tk, scale)
+    one_pass = B.chorus_block_mass(tq, tk, scale, lse=lse)
+    torch.cuda.synchronize()
+    mass_close(two_pass.cpu().numpy().astype(np.float64), ref)
+    mass_close(one_pass.cpu().numpy().astype(np.float64), ref)
+
+
+def test_attention_lse_of_a_sparse_mask_with_an_empty_row():
+    cfg = W.scaled(W.CFG1, H=2)
+    Q, K, V = W.qkv_bits(cfg)
+    keep = W.unpack_bits(W.layer_mask(cfg), cfg.nk)
+    keep[1, 3, :] = False                                                  # empty row: lse = -inf, O = 0
+    bm = W.pack_bits(keep)
+    rp, ci = B.chorus_mask_to_index(torch.from_numpy(bm[None].view(np.int32)).to(dev()), cfg.nk)
+    lse = torch.zeros((1, cfg.H, cfg.N), dtype=torch.float32, device=dev())
+    B.chorus_block_sparse_attn_fwd(dbf16(Q), dbf16(K), dbf16(V), rp, ci, cfg.scale, lse=lse)
+    torch.cuda.synchronize()
+    items = np.array([(0, 1, 3), (0, 0, 0), (0, 1, cfg.nq - 1)], np.int32)
+    _, lse_o = oracle.block_sparse_attn(Q, K, V, bm, cfg.scale, items=items, return_lse=True)
+    got = lse.cpu().numpy().astype(np.float64)
+    assert np.all(np.isneginf(got[0, 1, 3 * 128: 4 * 128])) and np.all(np.isneginf(lse_o[0]))
+    for t in (1, 2):
+        _, h, qb = items[t]
+        assert np.abs(got[0, h, 128 * qb: 128 * qb + 128] - lse_o[t]).max() <= 2e-3

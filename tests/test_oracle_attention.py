@@ -223,3 +223,26 @@ def test_strided_layout_bhnd_matches_bnhd():
     assert tq.strides != Q.strides
     O2 = run_oracle(tq, tk, tv, keep)
     assert np.array_equal(O, O2)
+
+
+def test_row_log_sum_exp_matches_scipy():
+    # full mask: lse_i = logsumexp_j(scale * q_i . k_j) over all keys (a library routine);
+    # a pruned mask: the same over the retained keys only; empty row: -inf
+    from scipy.special import logsumexp
+    N, H, scale = 200, 2, 0.11
+    Q, K, V = random_qkv_bits(N, H, seed=21)
+    nq, nk = 2, 4
+    q, k = bits_to_f64(Q), bits_to_f64(K)
+    keep = np.ones((H, nq, nk), dtype=bool)
+    keep[1, 0, 1:3] = False
+    keep[1, 1, :] = False                                     # an empty query-block row
+    items = np.array([(0, h, qb) for h in range(H) for qb in range(nq)], np.int32)
+    _, lse = oracle.block_sparse_attn(Q, K, V, W.pack_bits(keep), scale, items=items, return_lse=True)
+    for t, (_, h, qb) in enumerate(items):
+        rows = range(qb * 128, min(N, qb * 128 + 128))
+        cols = np.repeat(keep[h, qb], 64)[:N]
+        for r, i in enumerate(rows):
+            s = scale * (k[0, cols, h] @ q[0, i, h])
+            want = logsumexp(s) if cols.any() else -np.inf
+            assert (lse[t, r] == want) if not cols.any() else abs(lse[t, r] - want) < 1e-12
+        assert np.all(np.isneginf(lse[t, len(rows):]))        # rows beyond N
