@@ -47,7 +47,7 @@ typedef enum {
     CHORUS_ERR_CUDA = 4         /* a CUDA call failed; see chorus_last_error()              */
 } chorus_status;
 
-typedef enum { CHORUS_BF16 = 0, CHORUS_FP8_E4M3 = 1 } chorus_dtype;
+typedef enum { CHORUS_BF16 = 0, CHORUS_FP8_E4M3 = 1, CHORUS_FP16 = 2 } chorus_dtype;
 
 /* ---------------------------------------------------------------------------------------------
  * Mask decode ("stored, indexed by denoising step, transformer layer, and attention
@@ -114,7 +114,8 @@ typedef struct {
     const float* v_scale; /* [B][H][d]           */
 } chorus_fp8_scales;
 
-/* Q, K, V   device; dtype BF16: bf16 elements; dtype FP8_E4M3: e4m3 (fn) codes.  Base pointers
+/* Q, K, V   device; dtype BF16: bf16 elements; dtype FP16: IEEE half elements (the paper's
+ *           non-quantised path); dtype FP8_E4M3: e4m3 (fn) codes.  Base pointers
  *           16-byte aligned; strides multiples of 8 (bf16) / 16 (fp8) elements (TMA rules).
  * row_ptr   device, int32, points at THIS layer's first row: H*nq_blk + 1 readable entries,
  *           nq_blk = ceil(N/128); the same mask is used for every b.
@@ -122,10 +123,11 @@ typedef struct {
  *           lie in [0, ceil(N/64)) and ascend within a row (what chorus_mask_to_index produces);
  *           anything else is undefined behaviour.
  * scale     multiplies QK^T before the softmax (1/sqrt(128) in all workloads).
- * O         device, bf16 for both dtypes, 16-byte aligned, strides multiples of 8 elements.
- * fp8       NULL iff dtype == CHORUS_BF16.
+ * O         device, bf16 for dtype BF16 and FP8_E4M3, fp16 for dtype FP16; 16-byte aligned, strides
+ *           multiples of 8 elements.
+ * fp8       non-NULL iff dtype == CHORUS_FP8_E4M3.
  * Accuracy against the fp64 oracle on the same input bytes (BASELINE.json north_star):
- *           BF16: max|err| <= 2e-2, mean|err| <= 2e-3;  FP8: max|err| <= 8e-2, cosine >= 0.995.
+ *           BF16 and FP16: max|err| <= 2e-2, mean|err| <= 2e-3;  FP8: max|err| <= 8e-2, cosine >= 0.995.
  * Errors: INVALID_ARG (null pointer, misalignment, bad strides, N/H/B <= 0, fp8/dtype mismatch),
  *         UNSUPPORTED (d != 128, unknown dtype), CUDA.
  */

@@ -27,6 +27,8 @@ def lib():
         _lib.oracle_mask_to_index.restype = C.c_int64
         _lib.oracle_e4m3_to_double.restype = C.c_double
         _lib.oracle_e4m3_to_double.argtypes = [C.c_uint8]
+        _lib.oracle_f16_to_double.restype = C.c_double
+        _lib.oracle_f16_to_double.argtypes = [C.c_uint16]
         _lib.oracle_float_to_e4m3.restype = C.c_uint8
         _lib.oracle_float_to_e4m3.argtypes = [C.c_float]
         _lib.oracle_num_threads.restype = C.c_int
@@ -72,14 +74,14 @@ def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_th
                       return_weight_sum=False, return_lse=False):
     """fp64 block-sparse attention on the exact input bytes.
 
-    Q, K, V: [B][N][H][d] numpy arrays, uint16 (bf16 bits) or uint8 (e4m3 codes; then
+    Q, K, V: [B][N][H][d] numpy arrays, uint16 (bf16 bits), float16, or uint8 (e4m3 codes; then
     fp8_scales = (q_scale [B][H][ceil(N/128)], k_scale same, v_scale [B][H][d]) float32).
     bitmask: uint32 [H][nq][words] (one layer).  items: int array [n][3] of (b, h, qb); default all.
     Returns out float64 [n_items][128][d] (rows beyond N are 0)  (+ weight sums [n_items][128])
     (+ row log-sum-exp [n_items][128], natural log, -inf for empty rows, if return_lse).
     """
-    assert Q.dtype == K.dtype == V.dtype and Q.dtype in (np.uint16, np.uint8)
-    dtype = 0 if Q.dtype == np.uint16 else 1
+    assert Q.dtype == K.dtype == V.dtype and Q.dtype in (np.uint16, np.uint8, np.float16)
+    dtype = {np.dtype(np.uint16): 0, np.dtype(np.uint8): 1, np.dtype(np.float16): 2}[Q.dtype]
     B, N, H, d = Q.shape
     nq, nk = (N + BQ - 1) // BQ, (N + BK - 1) // BK
     bm = _c(bitmask, np.uint32)
@@ -93,7 +95,7 @@ def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_th
     out = np.zeros((n, BQ, d), dtype=np.float64)
     ws = np.zeros((n, BQ), dtype=np.float64) if return_weight_sum else None
     lse = np.zeros((n, BQ), dtype=np.float64) if return_lse else None
-    if dtype:
+    if dtype == 1:
         qs, ks, vs = (_c(x, np.float32) for x in fp8_scales)
         nsb = (N + 127) // 128
         assert qs.size == B * H * nsb and ks.size == B * H * nsb and vs.size == B * H * d
@@ -134,6 +136,10 @@ def quantize_fp8(Q, K, V):
 
 def e4m3_to_double(code: int) -> float:
     return float(lib().oracle_e4m3_to_double(int(code)))
+
+
+def f16_to_double(bits: int) -> float:
+    return float(lib().oracle_f16_to_double(int(bits)))
 
 
 def float_to_e4m3(x: float) -> int:

@@ -51,6 +51,16 @@ inline double bf16_to_double(uint16_t b) {
     return static_cast<double>(f);
 }
 
+// IEEE binary16 -> double: 1 sign, 5 exponent (bias 15), 10 mantissa; subnormals m/1024 * 2^-14.
+inline double f16_to_double(uint16_t hbits) {
+    const int sign = (hbits >> 15) & 1, e = (hbits >> 10) & 0x1F, m = hbits & 0x3FF;
+    double v;
+    if (e == 0x1F) v = m ? std::numeric_limits<double>::quiet_NaN() : std::numeric_limits<double>::infinity();
+    else if (e == 0) v = std::ldexp(static_cast<double>(m) / 1024.0, -14);
+    else v = std::ldexp(1.0 + static_cast<double>(m) / 1024.0, e - 15);
+    return sign ? -v : v;
+}
+
 // e4m3fn -> double.  1 sign, 4 exponent (bias 7), 3 mantissa; no infinities; S.1111.111 is NaN;
 // largest finite 448 = 1.75 * 2^8; subnormals m/8 * 2^-6.
 inline double e4m3_to_double(uint8_t c) {
@@ -138,7 +148,8 @@ int64_t oracle_mask_to_index(const uint32_t* bitmask, int L, int H, int nq, int 
 //     s_j  = scale * sum_c Q[i,h,c] K[j,h,c]
 //     m = max_j s_j ;  p_j = exp(s_j - m) ;  l = sum_j p_j
 //     O[i,h,:] = (sum_j p_j V[j,h,:]) / l                  J(i) empty => O = 0 (R7)
-// Everything in fp64 on the exact values of the input bytes.  dtype 0: bf16 bits; dtype 1: e4m3
+// Everything in fp64 on the exact values of the input bytes.  dtype 0: bf16 bits; dtype 2: IEEE
+// binary16 bits (the paper's non-quantised path); dtype 1: e4m3
 // codes dequantised as code * scale (q_scale[b][h][i/128], k_scale[b][h][j/128], v_scale[b][h][c];
 // R10).  The oracle reads the BITMASK, never a CSR, so a decode bug cannot hide.
 //
@@ -179,6 +190,7 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
             // exact value of one input element as a double (dequantised for FP8, R10)
             auto load = [&](const void* base, int64_t off, double sc) -> double {
                 if (dtype == 0) return bf16_to_double(static_cast<const uint16_t*>(base)[off]);
+                if (dtype == 2) return f16_to_double(static_cast<const uint16_t*>(base)[off]);
                 return e4m3_to_double(static_cast<const uint8_t*>(base)[off]) * sc;
             };
             // J = retained, valid keys of this query block (the same set for its 128 rows)
@@ -192,10 +204,10 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
             Vd.resize(nj * d);
             for (size_t x = 0; x < nj; ++x) {
                 const int j = js[x];
-                const double ks = dtype ? static_cast<double>(
+                const double ks = dtype == 1 ? static_cast<double>(
                     k_scale[(static_cast<int64_t>(b) * H + h) * nsb + j / 128]) : 1.0;
                 for (int c = 0; c < d; ++c) {
-                    const double vs = dtype ? static_cast<double>(
+                    const double vs = dtype == 1 ? static_cast<double>(
                         v_scale[(static_cast<int64_t>(b) * H + h) * d + c]) : 1.0;
                     Kd[x * d + c] = load(K, b * k_sb + j * k_sn + h * k_sh + c, ks);
                     Vd[x * d + c] = load(V, b * v_sb + j * v_sn + h * v_sh + c, vs);
@@ -211,7 +223,7 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
                 if (lse) lse[static_cast<int64_t>(t) * BQ + r] = -std::numeric_limits<double>::infinity();
                 if (i >= N || nj == 0) continue;
 
-                const double qs = dtype ? static_cast<double>(
+                const double qs = dtype == 1 ? static_cast<double>(
                     q_scale[(static_cast<int64_t>(b) * H + h) * nsb + i / 128]) : 1.0;
                 for (int c = 0; c < d; ++c) q[c] = load(Q, b * q_sb + i * q_sn + h * q_sh + c, qs);
 
@@ -300,6 +312,7 @@ void oracle_quantize_fp8(const uint16_t* Q, const uint16_t* K, const uint16_t* V
 
 // Element-wise helpers exposed so the tests can pin the two conversions on their own.
 double oracle_e4m3_to_double(uint8_t code) { return e4m3_to_double(code); }
+double oracle_f16_to_double(uint16_t bits) { return f16_to_double(bits); }
 uint8_t oracle_float_to_e4m3(float x) { return float_to_e4m3_rne_sat(x); }
 
 // -------------------------------------------------------------------------------------------------

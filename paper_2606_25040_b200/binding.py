@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libchorus.so")
 
 CHORUS_OK, CHORUS_ERR_INVALID_ARG, CHORUS_ERR_UNSUPPORTED, CHORUS_ERR_CAPACITY, CHORUS_ERR_CUDA = range(5)
-CHORUS_BF16, CHORUS_FP8_E4M3 = 0, 1
+CHORUS_BF16, CHORUS_FP8_E4M3, CHORUS_FP16 = 0, 1, 2
 BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
 
 EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
@@ -170,8 +170,11 @@ def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype:
     row_ptr: this layer's H*nq+1 entries (a view into the full row_ptr is fine).  Returns O (bf16)."""
     assert Q.is_cuda and K.is_cuda and V.is_cuda
     B, N, H, d = Q.shape
+    if Q.dtype == torch.float16:          # the paper's non-quantised path (PAPER.md:L97): fp16 in, fp16 out
+        dtype = CHORUS_FP16
     if O is None:
-        O = torch.empty((B, N, H, d), dtype=torch.bfloat16, device=Q.device)
+        O = torch.empty((B, N, H, d), dtype=torch.float16 if dtype == CHORUS_FP16 else torch.bfloat16,
+                        device=Q.device)
     shape = attn_shape(Q, K, V, O)
     sc = None
     if fp8_scales is not None:

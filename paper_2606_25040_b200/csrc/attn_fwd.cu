@@ -23,6 +23,9 @@
 // row sums, normalises, converts to bf16, stages in shared memory and writes with TMA stores
 // (coalesced 128-byte rows; rows beyond N are clipped by the tensor map).
 //
+// FP16 variant (template kF16; "for the non-quantized (fp16) path"): fp16 Q / K / V, P
+// and O; the same pipeline with the kind::f16 operand format switched.
+//
 // FP8 variant (template kFp8; R10-R12): e4m3 Q / K / V tiles (one 128-byte row holds all
 // 128 channels), tcgen05.mma kind::f8f6f4 with fp32 accumulation, V again an MN-major B operand,
 // P cast to e4m3 after a 2^5 shift, the Q / K block scales folded into the exp2 constant of each
@@ -151,7 +154,7 @@ __device__ __forceinline__ float max64(const uint32_t* sv) {
     return fmaxf(fmaxf(a0, a1), fmaxf(a2, a3));
 }
 
-template <bool kFp8>
+template <bool kFp8, bool kF16>   // e4m3 inputs / fp16 inputs and output (neither: bf16)
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmO,
@@ -258,7 +261,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             }
         } else if (warp == MMA_WARP) {
             // kind::f16: format 1 = bf16; kind::f8f6f4: format 0 = e4m3.  PV: B (= V) is MN-major.
-            constexpr uint32_t FMT = kFp8 ? 0u : 1u;
+            constexpr uint32_t FMT = (kFp8 || kF16) ? 0u : 1u;   // kind::f16: 0 = fp16, 1 = bf16
             constexpr uint32_t IDESC_S128 = make_idesc(FMT, FMT, 128, 128, 0, 0);
             constexpr uint32_t IDESC_S64 = make_idesc(FMT, FMT, 128, 64, 0, 0);
             constexpr uint32_t IDESC_PV = make_idesc(FMT, FMT, 128, 128, 0, 1);
@@ -521,7 +524,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             for (int k = 0; k < 16; ++k) {
                                 const float2 pp = exp_pair(k);
                                 lacc = fadd2(lacc, pp);
-                                pk[k] = pack_bf16x2(pp.x, pp.y);
+                                pk[k] = kF16 ? pack_f16x2(pp.x, pp.y) : pack_bf16x2(pp.x, pp.y);
                             }
                             tmem_st16(tS + c * 16, pk);      // P: bf16 pairs over the first 64 S columns
                         }
@@ -618,8 +621,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         x0 = __uint_as_float(o[4 * k4]) * w.x;     x1 = __uint_as_float(o[4 * k4 + 1]) * w.y;
                         x2 = __uint_as_float(o[4 * k4 + 2]) * w.z; x3 = __uint_as_float(o[4 * k4 + 3]) * w.w;
                     }
-                    pk[2 * k4] = pack_bf16x2(x0, x1);
-                    pk[2 * k4 + 1] = pack_bf16x2(x2, x3);
+                    pk[2 * k4] = kF16 ? pack_f16x2(x0, x1) : pack_bf16x2(x0, x1);
+                    pk[2 * k4 + 1] = kF16 ? pack_f16x2(x2, x3) : pack_bf16x2(x2, x3);
                 }
 #pragma unroll
                 for (int q4 = 0; q4 < 4; ++q4) {
@@ -659,18 +662,18 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 }  // namespace
 
-template <bool kFp8>
+template <bool kFp8, bool kF16>
 static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                               const CUtensorMap& tmO, const AttnParams& p, cudaStream_t stream) {
     constexpr uint32_t smem = Cfg<kFp8>::SMEM_BYTES;
-    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kFp8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kFp8, kF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     const int n_items = p.B * p.H * p.nq;
     const int grid = n_items < sms ? n_items : sms;
-    attn_fwd_kernel<kFp8><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
+    attn_fwd_kernel<kFp8, kF16><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
     count_launch(1);
     return cudaGetLastError();
 }
@@ -678,8 +681,9 @@ static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, co
 cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
                             cudaStream_t stream) {
-    if (dtype == CHORUS_BF16) return launch_one<false>(tmQ, tmK, tmV, tmO, p, stream);
-    if (dtype == CHORUS_FP8_E4M3) return launch_one<true>(tmQ, tmK, tmV, tmO, p, stream);
+    if (dtype == CHORUS_BF16) return launch_one<false, false>(tmQ, tmK, tmV, tmO, p, stream);
+    if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false>(tmQ, tmK, tmV, tmO, p, stream);
+    if (dtype == CHORUS_FP16) return launch_one<false, true>(tmQ, tmK, tmV, tmO, p, stream);
     return cudaErrorNotSupported;
 }
 

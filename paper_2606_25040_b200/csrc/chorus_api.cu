@@ -181,7 +181,7 @@ chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, con
                                                const chorus_fp8_scales* fp8, float* lse,
                                                void* cuda_stream) {
     g_err[0] = 0;
-    if (dtype != CHORUS_BF16 && dtype != CHORUS_FP8_E4M3)
+    if (dtype != CHORUS_BF16 && dtype != CHORUS_FP8_E4M3 && dtype != CHORUS_FP16)
         return set_error(CHORUS_ERR_UNSUPPORTED, "unknown dtype %d", static_cast<int>(dtype));
     if (!Q || !K || !V || !O || !row_ptr || !col_idx)
         return set_error(CHORUS_ERR_INVALID_ARG, "Q, K, V, O, row_ptr, col_idx must be non-null");
@@ -191,7 +191,7 @@ chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, con
         return set_error(CHORUS_ERR_INVALID_ARG, "fp8 scales must be given iff dtype is FP8_E4M3");
     if (fp8 && (!fp8->q_scale || !fp8->k_scale || !fp8->v_scale))
         return set_error(CHORUS_ERR_INVALID_ARG, "fp8 scale pointers must be non-null");
-    const int eb = dtype == CHORUS_BF16 ? 2 : 1;
+    const int eb = dtype == CHORUS_FP8_E4M3 ? 1 : 2;
     chorus_status st = validate_shape(shape, 16 / eb, true);
     if (st != CHORUS_OK) return st;
     const chorus_attn_shape& s = *shape;

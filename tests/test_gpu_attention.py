@@ -177,3 +177,27 @@ def test_density_sweep_one_head():
         bm = W.layer_mask(cfg, density=rho)
         items = sample_items(1, cfg.nq, 3, seed=int(rho * 100), always=[(0, 0, cfg.nq - 1)])
         compare(cfg, Q, K, V, bm, items)
+
+
+def _fp16_inputs(cfg, seed):
+    g = np.random.default_rng(seed)
+    return tuple(g.standard_normal((cfg.B, cfg.N, cfg.H, cfg.d)).astype(np.float16) for _ in range(3))
+
+
+@pytest.mark.parametrize("cfg,n_items", [(W.CFG1, None), (W.scaled(W.CFG2, H=2), 6)], ids=["cfg1", "480p-2heads"])
+def test_fp16_path_matches_oracle(cfg, n_items):
+    # dtype CHORUS_FP16 (the non-quantised path is fp16): fp16 Q/K/V, fp16 O
+    Q, K, V = _fp16_inputs(cfg, 77)
+    bm = W.layer_mask(cfg)
+    rp, ci = B.chorus_mask_to_index(dmask(bm[None]), cfg.nk)
+    t = lambda x: torch.from_numpy(x).to("cuda:0")
+    O = B.chorus_block_sparse_attn_fwd(t(Q), t(K), t(V), rp, ci, cfg.scale)
+    torch.cuda.synchronize()
+    assert O.dtype == torch.float16
+    O = O.float().cpu().numpy().astype(np.float64)
+    items = all_items(cfg.H, cfg.nq) if n_items is None else sample_items(cfg.H, cfg.nq, n_items, seed=3,
+                                                                          always=[(0, cfg.H - 1, cfg.nq - 1)])
+    ref = oracle_items(Q, K, V, bm, cfg.scale, items)
+    mx, mean, relfro, _ = err_stats(gather_items(O, items, cfg.N), ref)
+    assert mx <= BF16_MAX and mean <= BF16_MEAN, (mx, mean)
+    assert mx <= BF16_MAX_TIGHT and relfro <= BF16_RELFRO, (mx, relfro)

@@ -246,3 +246,25 @@ def test_row_log_sum_exp_matches_scipy():
             want = logsumexp(s) if cols.any() else -np.inf
             assert (lse[t, r] == want) if not cols.any() else abs(lse[t, r] - want) < 1e-12
         assert np.all(np.isneginf(lse[t, len(rows):]))        # rows beyond N
+
+
+def test_fp16_input_conversion_matches_numpy_for_every_bit_pattern():
+    bits = np.arange(65536, dtype=np.uint16)
+    want = bits.view(np.float16).astype(np.float64)
+    got = np.array([oracle.f16_to_double(int(b)) for b in bits])
+    nan = np.isnan(want)
+    assert np.array_equal(np.isnan(got), nan) and np.array_equal(got[~nan], want[~nan])
+
+
+def test_fp16_attention_equals_dense_numpy():
+    # the paper's non-quantised path is fp16: same definition, fp16 input bytes
+    N, H, scale = 200, 2, 0.1
+    g = np.random.default_rng(4)
+    Q, K, V = (g.standard_normal((1, N, H, 128)).astype(np.float16) for _ in range(3))
+    full = W.pack_bits(np.ones((H, 2, 4), dtype=bool))
+    items = np.array([(0, h, qb) for h in range(H) for qb in range(2)], np.int32)
+    out = oracle.scatter_items(oracle.block_sparse_attn(Q, K, V, full, scale, items=items), items, N, H)
+    for h in range(H):
+        ref = dense_softmax_attention(Q[0, :, h].astype(np.float64), K[0, :, h].astype(np.float64),
+                                      V[0, :, h].astype(np.float64), scale)
+        assert np.allclose(out[0, :, h], ref, rtol=1e-12, atol=1e-14)
