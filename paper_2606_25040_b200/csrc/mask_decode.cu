@@ -21,7 +21,10 @@ namespace {
 
 constexpr int DEC_THREADS = 256;
 constexpr int DEC_WARPS = DEC_THREADS / 32;
-constexpr int SUBTILES = 4;
+#ifndef CHORUS_DEC_SUBTILES
+#define CHORUS_DEC_SUBTILES 4
+#endif
+constexpr int SUBTILES = CHORUS_DEC_SUBTILES;
 constexpr int TILE_WORDS = DEC_THREADS * SUBTILES;   // 1024 words = up to 32768 key blocks
 constexpr int STAGE = DEC_THREADS * 32;              // one sub-tile can never hold more entries
 
@@ -98,12 +101,29 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
         sub_total[sidx] = tot;
         tile_total += tot;
     }
+    // a tile whose entries all fit the staging buffer is expanded in one go (the usual case)
+    const bool fast = col_idx != nullptr && tile_total <= STAGE;
     // 2c. decoupled look-back, 256 predecessor tiles per step (thread i looks at tile look - i): with
     // a thousand tiles in flight the nearest tile that already knows its prefix is that far back
     {
         unsigned long long* mine = status + 1 + tile;
         if (threadIdx.x == 0)
             st_status(mine, (tile == 0 ? ST_INC : ST_AGG) | static_cast<uint32_t>(tile_total));
+        // While the predecessors publish, expand: the staging offsets do not need the global base.
+        if (fast) {
+#pragma unroll
+            for (int sidx = 0; sidx < SUBTILES; ++sidx) {
+                uint32_t x = v[sidx];
+                const int kb0 = win[sidx] * 32;
+                int e = off[sidx];
+                while (x) {
+                    const int b = __ffs(x) - 1;
+                    x &= x - 1;
+                    s_stage[e + (e >> 5)] = kb0 + b;
+                    ++e;
+                }
+            }
+        }
         int base = 0;
         for (int look = tile - 1; tile > 0;) {
             const int t = look - static_cast<int>(threadIdx.x);
@@ -141,7 +161,12 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
         if (w == n_words - 1) row_ptr[rows] = static_cast<int32_t>(base + tile_total);
     }
     if (col_idx == nullptr) return;
-    // 3b. expand sub-tile by sub-tile through the staging buffer
+    if (fast) {     // staged before the look-back; the __syncthreads after it ordered the writes
+        for (int t = threadIdx.x; t < tile_total; t += DEC_THREADS)
+            if (base + t < col_cap) col_idx[base + t] = s_stage[t + (t >> 5)];
+        return;
+    }
+    // 3b. a fuller tile: expand sub-tile by sub-tile through the staging buffer
     int sub0 = 0;
 #pragma unroll
     for (int sidx = 0; sidx < SUBTILES; ++sidx) {
