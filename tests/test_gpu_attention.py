@@ -201,3 +201,25 @@ def test_fp16_path_matches_oracle(cfg, n_items):
     mx, mean, relfro, _ = err_stats(gather_items(O, items, cfg.N), ref)
     assert mx <= BF16_MAX and mean <= BF16_MEAN, (mx, mean)
     assert mx <= BF16_MAX_TIGHT and relfro <= BF16_RELFRO, (mx, relfro)
+
+
+def test_tail_probe_padded_allocation_does_not_leak():
+    # K / V live in an allocation padded beyond N whose extra rows hold huge
+    # values and NaNs; the kernel sees N through the shape only.  Nothing of the padding may leak:
+    # the result must be bit-identical to the run on an unpadded copy.
+    cfg = W.scaled(W.CFG2, H=2, frames=2)            # N = 3120: last key block 48 keys, last q block 48 rows
+    Q, K, V = W.qkv_bits(cfg)
+    bm = W.layer_mask(cfg)
+    rp, ci = B.chorus_mask_to_index(dmask(bm[None]), cfg.nk)
+    q, k, v = dbf16(Q), dbf16(K), dbf16(V)
+    O_ref = B.chorus_block_sparse_attn_fwd(q, k, v, rp, ci, cfg.scale)
+    pad = 256
+    def padded(t, fill):
+        buf = torch.full((1, cfg.N + pad, cfg.H, cfg.d), fill, dtype=torch.bfloat16, device=t.device)
+        buf[:, : cfg.N] = t
+        return buf[:, : cfg.N]                        # a view: same strides, the padding sits right behind it
+    O_pad = B.chorus_block_sparse_attn_fwd(padded(q, 3e4), padded(k, float("nan")), padded(v, -3e38), rp, ci,
+                                           cfg.scale)
+    torch.cuda.synchronize()
+    assert not torch.isnan(O_pad.float()).any()
+    assert torch.equal(O_ref, O_pad)
