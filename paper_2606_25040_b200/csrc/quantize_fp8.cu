@@ -70,8 +70,10 @@ __device__ __forceinline__ uint2 quant8(const uint4& u, const Divisor& s) {
 }
 
 // grid: (H, nsb, 2*B), heads fastest so that the CTAs in flight together cover whole 128-token
-// slabs of the [N][H][d] tensor (contiguous DRAM pages); blockIdx.z = 2*b + which (0: Q, 1: K)
-__global__ void __launch_bounds__(QT)
+// slabs of the [N][H][d] tensor (contiguous DRAM pages); blockIdx.z = 2*b + which (0: Q, 1: K).
+// The tile is read twice (amax, then cast; the second read comes from L1/L2) instead of being held
+// in registers: 32 registers per thread, eight CTAs per SM instead of four.
+__global__ void __launch_bounds__(QT, 8)
 qk_quantize_kernel(const uint16_t* __restrict__ Q, const uint16_t* __restrict__ K,
                    chorus_attn_shape s, uint8_t* __restrict__ q8, uint8_t* __restrict__ k8,
                    float* __restrict__ q_scale, float* __restrict__ k_scale, int nsb) {
@@ -86,18 +88,13 @@ qk_quantize_kernel(const uint16_t* __restrict__ Q, const uint16_t* __restrict__ 
     float* S = which ? k_scale : q_scale;
 
     const int sub = threadIdx.x & 15, rowp = threadIdx.x >> 4;
-    Tile t;
+    const uint4* src = reinterpret_cast<const uint4*>(X + b * sb + (static_cast<int64_t>(blk) * 128 + rowp) * sn + h * sh) + sub;
+    const int64_t step = 16 * sn / 8;                 // 16 token rows further, in uint4 units
+    const int rows_left = s.N - blk * 128 - rowp;     // this thread's rows: rowp, rowp + 16, ... while < rows_left
     float m = 0.f;
 #pragma unroll
-    for (int p = 0; p < 8; ++p) {
-        const int n = blk * 128 + p * 16 + rowp;
-        if (n < s.N) {
-            t.v[p] = __ldg(reinterpret_cast<const uint4*>(X + b * sb + n * sn + h * sh) + sub);
-            m = fmaxf(m, amax8(t.v[p]));
-        } else {
-            t.v[p] = make_uint4(0, 0, 0, 0);
-        }
-    }
+    for (int p = 0; p < 8; ++p)
+        if (p * 16 < rows_left) m = fmaxf(m, amax8(__ldg(src + p * step)));
     for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
     if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = m;
     __syncthreads();
@@ -110,14 +107,11 @@ qk_quantize_kernel(const uint16_t* __restrict__ Q, const uint16_t* __restrict__ 
     }
     __syncthreads();
     const Divisor sc = make_divisor(s_scale);
+    uint2* dst = reinterpret_cast<uint2*>(X8 + ((static_cast<int64_t>(b) * s.N + blk * 128 + rowp) * s.H + h) * 128) + sub;
+    const int64_t dstep = 16 * static_cast<int64_t>(s.H) * 128 / 8;
 #pragma unroll
-    for (int p = 0; p < 8; ++p) {
-        const int n = blk * 128 + p * 16 + rowp;
-        if (n < s.N) {
-            uint8_t* dst = X8 + ((static_cast<int64_t>(b) * s.N + n) * s.H + h) * 128;
-            reinterpret_cast<uint2*>(dst)[sub] = quant8(t.v[p], sc);
-        }
-    }
+    for (int p = 0; p < 8; ++p)
+        if (p * 16 < rows_left) dst[p * dstep] = quant8(__ldg(src + p * step), sc);
 }
 
 // V column amax: grid (H, chunks, B); each CTA covers V_ROWS tokens; atomicMax on float bits
