@@ -40,3 +40,21 @@ def test_single_rank_is_identity_and_aggregate_scales_with_replicas():
     one = bench.whole_job_value(1, 5.5e12, 4.4)
     assert abs(one - 1250.0) < 1e-9
     assert bench.whole_job_value(8, 5.5e12, 4.4) == 8 * one      # weak scaling: same time, 8x the work
+
+
+def test_reference_arm_prints_the_contract_line():
+    # bench.py --impl reference: the oracle on the host cores, one JSON line with the base contract's keys
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "0", "--workload", "cfg1"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-500:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    for k in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+              "scaling", "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert k in line, k
+    assert line["impl"] == "reference" and line["dtype"] == "f64" and line["vs_baseline"] is None
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["value"] > 0
