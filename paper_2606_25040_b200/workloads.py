@@ -277,3 +277,30 @@ def hash_fill_masks(shape_rows: int, words: int, nk: int, density: float, seed: 
     g = _rng(seed, 7)
     keep = g.random((shape_rows, nk)) < density
     return pack_bits(keep).reshape(shape_rows, words)
+
+
+# ------------------------------------------------------------------------------------------------
+# "similar requests" for the mask-construction path (Observation 1 / Fig. 4)
+# ------------------------------------------------------------------------------------------------
+def clustered_request(N: int, H: int, reassigned: float, noise_seed: int, structure_seed: int = 1,
+                      clusters: int = 8, strength: float = 0.7, d: int = 128):
+    """Q, K bf16 bits [1][N][H][d] whose attention is block-structured: every 64-token block belongs to
+    one of `clusters` clusters (per head), and a token's q and k are strength * its cluster's centre
+    plus N(0,1) noise, so that a query attends mostly to the key blocks of its own cluster.  Two
+    requests with the same structure_seed share centres and block assignment except for a fraction
+    `reassigned` of the blocks, which is what "similarity" means here: reassigned = 0 is the same
+    scene with fresh noise, 1 an unrelated one.  Stands in for the paper's similar I2V requests; no
+    arithmetic of the method lives here."""
+    g = _rng(structure_seed, 11)
+    centres = g.standard_normal((H, clusters, d))
+    assign = g.integers(0, clusters, size=(H, (N + 63) // 64))
+    g2 = _rng(noise_seed, 12)
+    flip = g2.random(assign.shape) < reassigned
+    assign = np.where(flip, g2.integers(0, clusters, size=assign.shape), assign)
+    Q = np.empty((1, N, H, d), dtype=np.float32)
+    K = np.empty((1, N, H, d), dtype=np.float32)
+    for h in range(H):
+        c = np.repeat(assign[h], 64)[:N]
+        Q[0, :, h] = strength * centres[h, c] + g2.standard_normal((N, d))
+        K[0, :, h] = strength * centres[h, c] + g2.standard_normal((N, d))
+    return bf16_bits_from_f32(Q), bf16_bits_from_f32(K)

@@ -165,3 +165,56 @@ def test_attention_lse_of_a_sparse_mask_with_an_empty_row():
     for t in (1, 2):
         _, h, qb = items[t]
         assert np.abs(got[0, h, 128 * qb: 128 * qb + 128] - lse_o[t]).max() <= 2e-3
+
+
+def test_cross_request_mask_reuse_end_to_end():
+    # The method end to end on the device (Fig. 4/5), synthetic similar requests:
+    # historical request: dense attention (+LSE) -> block mass -> top-p mask with a floor (cached);
+    # new request: decode the cached mask -> block-sparse attention; its coverage on the new request's
+    # own true mass falls as the requests grow apart, and matches the oracle's figure.
+    N, H, nk, scale = 2048, 2, 32, 1 / np.sqrt(128)
+    nq = N // 128
+    g = np.random.default_rng(3)
+    V = W.bf16_bits_from_f32(g.standard_normal((1, N, H, 128)).astype(np.float32))
+    full = torch.full((1, H, nq, 1), -1, dtype=torch.int32, device=dev())
+    rp_full, ci_full = B.chorus_mask_to_index(full, nk)
+
+    def dense_mass(Qb, Kb):
+        lse = torch.empty((1, H, N), dtype=torch.float32, device=dev())
+        O = B.chorus_block_sparse_attn_fwd(dbf16(Qb), dbf16(Kb), dbf16(V), rp_full, ci_full, scale, lse=lse)
+        return O, B.chorus_block_mass(dbf16(Qb), dbf16(Kb), scale, lse=lse)
+
+    Qs, Ks = W.clustered_request(N, H, 0.0, noise_seed=100)
+    _, src_mass = dense_mass(Qs, Ks)
+    src_mask, kept = B.chorus_mask_from_mass(src_mass[0], 0.9, 0.1)            # the cached artefact
+    torch.cuda.synchronize()
+    assert kept.float().mean().item() / nk < 0.5
+    src_mask_o, _ = oracle.mask_from_mass(oracle.block_mass(Qs, Ks, scale)[0].astype(np.float32), nk, F(0.9), F(0.1))
+    agree = (W.unpack_bits(src_mask.cpu().numpy().view(np.uint32), nk) == W.unpack_bits(src_mask_o, nk)).mean()
+    assert agree > 0.995            # masses differ in the last bits, so a few threshold blocks may differ
+
+    cov = []
+    for f in (0.0, 0.25, 1.0):
+        Qt, Kt = W.clustered_request(N, H, f, noise_seed=200)
+        O_dense, tgt_mass = dense_mass(Qt, Kt)
+        c = B.chorus_mask_coverage(tgt_mass[0], src_mask, nk).cpu().numpy()
+        c_o = oracle.mask_coverage(oracle.block_mass(Qt, Kt, scale)[0].astype(np.float32),
+                                   src_mask.cpu().numpy().view(np.uint32), nk)
+        assert np.abs(c - c_o).max() <= 2e-3
+        cov.append(float(c.mean()))
+        # the new request's attention under the reused mask, against the oracle with that mask
+        rp, ci = B.chorus_mask_to_index(src_mask[None], nk)
+        O = B.chorus_block_sparse_attn_fwd(dbf16(Qt), dbf16(Kt), dbf16(V), rp, ci, scale)
+        torch.cuda.synchronize()
+        items = np.array([(0, 0, 0), (0, 1, nq - 1)], np.int32)
+        ref = oracle.block_sparse_attn(Qt, Kt, V, src_mask.cpu().numpy().view(np.uint32), scale, items=items)
+        got = O.float().cpu().numpy().astype(np.float64)
+        for t, (_, h, qb) in enumerate(items):
+            assert np.abs(got[0, 128 * qb: 128 * qb + 128, h] - ref[t]).max() <= 2e-2
+        if f == 0.0:
+            # what reuse costs in output error when the mask fits: small next to dropping a third of the mass
+            err_fit = (O.float() - O_dense.float()).abs().mean().item()
+        if f == 1.0:
+            err_unrelated = (O.float() - O_dense.float()).abs().mean().item()
+    assert cov[0] >= 0.9 and cov[0] > cov[1] > cov[2] and cov[2] < 0.75
+    assert err_fit < 0.5 * err_unrelated

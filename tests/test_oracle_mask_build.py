@@ -146,3 +146,24 @@ def test_true_top_p_mask_of_a_dense_pass_end_to_end():
     bm, kept = oracle.mask_from_mass(mass, nk, 0.9, 0.0)
     cov = oracle.mask_coverage(mass, bm, nk)
     assert (cov >= 0.9 - 1e-6).all() and (kept <= nk).all() and (kept >= 1).all()
+
+
+def test_reused_mask_coverage_grows_with_request_similarity():
+    # PAPER.md:L73 (Observation 1, Fig. 4): a true-top-p mask taken from a similar request "still
+    # preserves most of the target's attention mass", and "the coverage grows monotonically as the input
+    # conditions of the two requests become more similar".  Synthetic stand-in: block-clustered requests
+    # that share all but a fraction of their block structure (workloads.clustered_request).
+    N, H, nk, scale = 1024, 2, 16, 1 / np.sqrt(128)
+    Qs, Ks = W.clustered_request(N, H, 0.0, noise_seed=100)
+    src_mass = oracle.block_mass(Qs, Ks, scale)[0].astype(np.float32)
+    src_mask, kept = oracle.mask_from_mass(src_mass, nk, 0.9, 0.1)
+    assert kept.mean() / nk < 0.5                                  # a genuinely sparse mask
+    assert (oracle.mask_coverage(src_mass, src_mask, nk) >= 0.9 - 1e-6).all()
+    cov = []
+    for f in (0.0, 0.1, 0.25, 0.5, 1.0):
+        Qt, Kt = W.clustered_request(N, H, f, noise_seed=200)
+        tgt_mass = oracle.block_mass(Qt, Kt, scale)[0].astype(np.float32)
+        cov.append(oracle.mask_coverage(tgt_mass, src_mask, nk).mean())
+    assert cov[0] >= 0.9                                           # same scene, fresh noise: like its own mask
+    assert all(a > b for a, b in zip(cov, cov[1:]))                # monotone in similarity
+    assert cov[-1] < 0.7                                           # an unrelated request loses a third of the mass
