@@ -10,12 +10,19 @@
  *   chorus_visit_refresh          block-pair visit refreshing over groups of layers            (L93 (1), L153)
  *   chorus_mask_to_index          stored block bitmask  ->  CSR of kept key blocks per query block (L81, L87)
  *   chorus_quantize_fp8           bf16 Q/K/V -> e4m3 + scales for the FP8 backend              (L97)
- *   chorus_block_sparse_attn_fwd  block-sparse attention forward, BF16 or FP8 e4m3             (L97)
+ *   chorus_block_sparse_attn_fwd  block-sparse attention forward, BF16, FP16 or FP8 e4m3       (L97)
+ *   chorus_block_sparse_attn_fwd_lse   the same, also writing the rows' log-sum-exp            (L87)
+ * and, for the historical request whose masks get cached, and for sequence-parallel groups:
+ *   chorus_block_mass / chorus_mask_from_mass / chorus_mask_coverage
+ *                                 dense attention mass per block -> top-p mask with a top-k floor
+ *                                 -> coverage                                                  (L73, L81, L93 (2))
+ *   chorus_head_costs / chorus_schedule_heads   per-head cost and greedy head -> rank schedule (L95, appendix A)
  *
  * Conventions (all entry points)
  *   - Plain C: pointers and sizes only.  "device" = pointer into CUDA device memory of the current
  *     device; "host" = ordinary host memory.  Every buffer is owned by the caller; the library
- *     allocates nothing that outlives a call, keeps no global state, and never frees caller memory.
+ *     allocates nothing that outlives a call, keeps no global state (beyond cached device attributes),
+ *     and never frees caller memory.
  *   - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream)
  *     and the call returns without synchronising.
  *   - Errors: an integer status, never an exception.  Argument errors are detected on the host
