@@ -3,14 +3,14 @@
 // Decode (PAPER.md:L81/L87/L93; include/chorus.h): packed block bitmask [rows][words] ->
 // CSR (row_ptr, col_idx), ascending inside each row.  ONE pass over the bitmask, one launch (plus a
 // memset of the small look-back array): the bitmask is taken as a flat array of rows*words words,
-// cut into tiles of 1024 words (four sub-tiles of 256, one word per thread each); a block
-//   1. loads its tile (coalesced), clears the pad bits of the last word of each row and counts;
+// cut into tiles of 256*WPT words, WPT consecutive words per thread; a block
+//   1. loads its tile, clears the pad bits of the last word of each row and counts;
 //   2. scans the counts inside the block and gets the number of set bits in front of its tile with
 //      a decoupled look-back over the per-tile status words, 256 at a time (tiles are taken in
 //      ticket order, so a tile only ever waits for tiles that already run);
-//   3. writes row_ptr for every row that begins in the tile, then, sub-tile by sub-tile, every
-//      thread walks the set bits of its word into a shared-memory staging buffer, which the block
-//      copies to col_idx in contiguous, coalesced runs.
+//   3. writes row_ptr for every row that begins in the tile; every thread walks the set bits of its
+//      words into a shared-memory staging buffer (before the look-back when the whole tile fits),
+//      which the block copies to col_idx in contiguous, coalesced runs.
 // Algorithmic traffic: 4*(rows*words) read + 4*(rows+1) + 4*nnz written; nothing is read twice.
 #include <algorithm>
 
@@ -19,14 +19,12 @@
 namespace chorus {
 namespace {
 
+#ifndef CHORUS_DEC_STAGE
+#define CHORUS_DEC_STAGE 9216
+#endif
 constexpr int DEC_THREADS = 256;
 constexpr int DEC_WARPS = DEC_THREADS / 32;
-#ifndef CHORUS_DEC_SUBTILES
-#define CHORUS_DEC_SUBTILES 4
-#endif
-constexpr int SUBTILES = CHORUS_DEC_SUBTILES;
-constexpr int TILE_WORDS = DEC_THREADS * SUBTILES;   // 1024 words = up to 32768 key blocks
-constexpr int STAGE = DEC_THREADS * 32;              // one sub-tile can never hold more entries
+constexpr int STAGE = CHORUS_DEC_STAGE;                          // col_idx entries staged per round
 
 // per-tile status word: bits 63..62 = state (0 empty, 1 aggregate of the tile, 2 inclusive prefix),
 // low 32 bits = value.  Written and read with single 64-bit relaxed accesses.
@@ -41,6 +39,9 @@ __device__ __forceinline__ unsigned long long ld_status(const unsigned long long
     return v;
 }
 
+// WPT consecutive words per thread: 4 for large mask sets (fewer scans, divisions and status words per
+// word), 1 for a single layer (more, smaller tiles: one 480p layer is only 160 K words)
+template <int WPT>
 __global__ void __launch_bounds__(DEC_THREADS)
 decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, int words,
                     int32_t* __restrict__ row_ptr, int32_t* __restrict__ col_idx, int64_t col_cap,
@@ -48,9 +49,10 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
     // entry e sits at e + e/32: threads whose runs start 8, 16 or 32 entries apart (25 %, 50 %, full
     // density) then hit different banks when they all write their k-th entry
     __shared__ int32_t s_stage[STAGE + STAGE / 32];
-    __shared__ int s_warp[SUBTILES][DEC_WARPS];
+    __shared__ int s_warp[DEC_WARPS];
     __shared__ int2 s_look[DEC_WARPS];
     __shared__ int s_tile, s_base;
+    constexpr int TILE_WORDS = DEC_THREADS * WPT;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) s_tile = static_cast<int>(atomicAdd(status, 1ull));
     __syncthreads();
@@ -61,45 +63,38 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
     const int rem = nk - (words - 1) * 32;                      // valid bits of a row's last word
     const uint32_t last_mask = rem >= 32 ? 0xffffffffu : ((1u << rem) - 1u);
 
-    // 1. load (word tile0 + 256 s + thread for sub-tile s), mask the pad bits, count
-    uint32_t v[SUBTILES];
-    int win[SUBTILES], rowi[SUBTILES], cnt[SUBTILES], inc[SUBTILES];
+    // 1. load WPT consecutive words per thread, mask the pad bits, count
+    const uint32_t w0 = tile0 + threadIdx.x * WPT;              // this thread's first word
+    uint32_t v[WPT];
+    const uint32_t row0 = w0 / static_cast<uint32_t>(words);    // one division per thread and tile
+    const int win0 = static_cast<int>(w0 - row0 * static_cast<uint32_t>(words));
+    int cnt = 0;
+    {
+        int wr = win0;
 #pragma unroll
-    for (int sidx = 0; sidx < SUBTILES; ++sidx) {
-        const uint32_t w = tile0 + sidx * DEC_THREADS + threadIdx.x;
-        const uint32_t r = w / static_cast<uint32_t>(words);
-        const int wr = static_cast<int>(w - r * static_cast<uint32_t>(words));
-        uint32_t x = (w < n_words) ? __ldg(bitmask + w) : 0u;
-        if (wr == words - 1) x &= last_mask;
-        v[sidx] = x;
-        win[sidx] = wr;
-        rowi[sidx] = static_cast<int>(r);
-        cnt[sidx] = __popc(x);
-        // 2a. inclusive scan inside the warp
-        int t = cnt[sidx];
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int u = __shfl_up_sync(0xffffffffu, t, o);
-            if (lane >= o) t += u;
+        for (int i = 0; i < WPT; ++i) {
+            uint32_t x = (w0 + i < n_words) ? __ldg(bitmask + w0 + i) : 0u;
+            if (wr == words - 1) x &= last_mask;
+            v[i] = x;
+            cnt += __popc(x);
+            if (++wr == words) wr = 0;
         }
-        inc[sidx] = t;
-        if (lane == 31) s_warp[sidx][warp] = t;
     }
+    // 2a/2b. one exclusive scan of the thread counts inside the block
+    int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += u;
+    }
+    if (lane == 31) s_warp[warp] = inc;
     __syncthreads();
-    // 2b. offsets of this thread's four words inside the tile, and the tile total
-    int off[SUBTILES], sub_total[SUBTILES], tile_total = 0;
+    int off = inc - cnt, tile_total = 0;     // set bits of the tile in front of this thread's words
 #pragma unroll
-    for (int sidx = 0; sidx < SUBTILES; ++sidx) {
-        int before = 0, tot = 0;
-#pragma unroll
-        for (int w = 0; w < DEC_WARPS; ++w) {
-            const int u = s_warp[sidx][w];
-            if (w < warp) before += u;
-            tot += u;
-        }
-        off[sidx] = tile_total + before + inc[sidx] - cnt[sidx];
-        sub_total[sidx] = tot;
-        tile_total += tot;
+    for (int w = 0; w < DEC_WARPS; ++w) {
+        const int u = s_warp[w];
+        if (w < warp) off += u;
+        tile_total += u;
     }
     // a tile whose entries all fit the staging buffer is expanded in one go (the usual case)
     const bool fast = col_idx != nullptr && tile_total <= STAGE;
@@ -111,17 +106,18 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
             st_status(mine, (tile == 0 ? ST_INC : ST_AGG) | static_cast<uint32_t>(tile_total));
         // While the predecessors publish, expand: the staging offsets do not need the global base.
         if (fast) {
+            int e = off, wr = win0;
 #pragma unroll
-            for (int sidx = 0; sidx < SUBTILES; ++sidx) {
-                uint32_t x = v[sidx];
-                const int kb0 = win[sidx] * 32;
-                int e = off[sidx];
+            for (int i = 0; i < WPT; ++i) {
+                uint32_t x = v[i];
+                const int kb0 = wr * 32;
                 while (x) {
                     const int b = __ffs(x) - 1;
                     x &= x - 1;
                     s_stage[e + (e >> 5)] = kb0 + b;
                     ++e;
                 }
+                if (++wr == words) wr = 0;
             }
         }
         int base = 0;
@@ -154,11 +150,16 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
     __syncthreads();
     const int64_t base = s_base;
     // 3a. row_ptr of the rows that begin in this tile; the thread holding the last word writes the total
+    {
+        int o = off, wr = win0;
+        uint32_t r = row0;
 #pragma unroll
-    for (int sidx = 0; sidx < SUBTILES; ++sidx) {
-        const uint32_t w = tile0 + sidx * DEC_THREADS + threadIdx.x;
-        if (win[sidx] == 0 && w < n_words) row_ptr[rowi[sidx]] = static_cast<int32_t>(base + off[sidx]);
-        if (w == n_words - 1) row_ptr[rows] = static_cast<int32_t>(base + tile_total);
+        for (int i = 0; i < WPT; ++i) {
+            if (wr == 0 && w0 + i < n_words) row_ptr[r] = static_cast<int32_t>(base + o);
+            if (w0 + i == n_words - 1) row_ptr[rows] = static_cast<int32_t>(base + tile_total);
+            o += __popc(v[i]);
+            if (++wr == words) { wr = 0; ++r; }
+        }
     }
     if (col_idx == nullptr) return;
     if (fast) {     // staged before the look-back; the __syncthreads after it ordered the writes
@@ -166,25 +167,46 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
             if (base + t < col_cap) col_idx[base + t] = s_stage[t + (t >> 5)];
         return;
     }
-    // 3b. a fuller tile: expand sub-tile by sub-tile through the staging buffer
-    int sub0 = 0;
+    // 3b. a fuller tile (WPT > 1 only): WPT rounds of one word per thread, so that every thread walks
+    // in every round.  Round r takes words r*256 .. r*256+255 of the tile - at most 8192 entries, one
+    // contiguous run - and finds each word's offset in a table the owning threads wrote; the table
+    // sits behind the largest round in the staging buffer.
+    if constexpr (WPT > 1) {
+        constexpr int ROUND_MAX = DEC_THREADS * 32;
+        static_assert(ROUND_MAX + ROUND_MAX / 32 + TILE_WORDS <= STAGE + STAGE / 32,
+                      "staging buffer too small for a round plus the offset table");
+        int* s_woff = s_stage + ROUND_MAX + ROUND_MAX / 32;
+        {
+            int o = off;
 #pragma unroll
-    for (int sidx = 0; sidx < SUBTILES; ++sidx) {
-        uint32_t x = v[sidx];
-        const int kb0 = win[sidx] * 32;
-        int e = off[sidx] - sub0;
-        while (x) {
-            const int b = __ffs(x) - 1;
-            x &= x - 1;
-            s_stage[e + (e >> 5)] = kb0 + b;
-            ++e;
+            for (int i = 0; i < WPT; ++i) {
+                s_woff[threadIdx.x * WPT + i] = o;
+                o += __popc(v[i]);
+            }
         }
         __syncthreads();
-        const int64_t dst0 = base + sub0;
-        for (int t = threadIdx.x; t < sub_total[sidx]; t += DEC_THREADS)
-            if (dst0 + t < col_cap) col_idx[dst0 + t] = s_stage[t + (t >> 5)];
-        __syncthreads();
-        sub0 += sub_total[sidx];
+#pragma unroll 1
+        for (int r = 0; r < WPT; ++r) {
+            const int j = r * DEC_THREADS + threadIdx.x;
+            const int lo = s_woff[r * DEC_THREADS];
+            const int hi = r + 1 < WPT ? s_woff[(r + 1) * DEC_THREADS] : tile_total;
+            const uint32_t g = tile0 + j;
+            const int wr = static_cast<int>(g % static_cast<uint32_t>(words));
+            uint32_t x = g < n_words ? __ldg(bitmask + g) : 0u;
+            if (wr == words - 1) x &= last_mask;
+            int e = s_woff[j] - lo;
+            const int kb0 = wr * 32;
+            while (x) {
+                const int b = __ffs(x) - 1;
+                x &= x - 1;
+                s_stage[e + (e >> 5)] = kb0 + b;
+                ++e;
+            }
+            __syncthreads();
+            for (int t = threadIdx.x; t < hi - lo; t += DEC_THREADS)
+                if (base + lo + t < col_cap) col_idx[base + lo + t] = s_stage[t + (t >> 5)];
+            __syncthreads();
+        }
     }
 }
 
@@ -206,7 +228,13 @@ visit_refresh_kernel(uint32_t* __restrict__ bitmask, int n_groups, int64_t words
     }
 }
 
-inline int64_t n_tiles_for(int64_t rows, int words) { return (rows * words + TILE_WORDS - 1) / TILE_WORDS; }
+// one word per thread below this many words (a few layers), four above
+constexpr int64_t SMALL_WORDS = 1 << 20;
+inline int wpt_for(int64_t n_words) { return n_words < SMALL_WORDS ? 1 : 4; }
+inline int64_t n_tiles_for(int64_t rows, int words) {
+    const int64_t n = rows * words, tw = static_cast<int64_t>(DEC_THREADS) * wpt_for(n);
+    return (n + tw - 1) / tw;
+}
 
 }  // namespace
 
@@ -222,8 +250,12 @@ cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, in
     auto* status = reinterpret_cast<unsigned long long*>((reinterpret_cast<uintptr_t>(workspace) + 7) & ~uintptr_t(7));
     cudaError_t e = cudaMemsetAsync(status, 0, static_cast<size_t>(nt + 1) * sizeof(unsigned long long), stream);
     if (e != cudaSuccess) return e;
-    decode_tiles_kernel<<<static_cast<unsigned>(nt), DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr,
-                                                                             col_idx, col_cap, status);
+    if (wpt_for(rows * words) == 1)
+        decode_tiles_kernel<1><<<static_cast<unsigned>(nt), DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr,
+                                                                                    col_idx, col_cap, status);
+    else
+        decode_tiles_kernel<4><<<static_cast<unsigned>(nt), DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr,
+                                                                                    col_idx, col_cap, status);
     count_launch(1);
     return cudaGetLastError();
 }

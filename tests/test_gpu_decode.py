@@ -69,6 +69,33 @@ def test_multi_layer_mask_set_and_count_only_and_capacity():
     assert np.array_equal(got[:cap], ci_o[:cap]) and np.all(got[cap:] == -7)
 
 
+def test_large_mask_set_four_words_per_thread():
+    """>= 2^20 words selects the 4-words-per-thread instantiation; row densities from 0 to 1 in
+    runs of uneven length put sparse (single pass) and full (four rounds) tiles next to each other, nk = 1182
+    leaves a 30-bit last word with garbage above it, and the word count is no multiple of the tile."""
+    L, H, nq, nk = 8, 8, 513, 1182
+    g = np.random.default_rng(20260)
+    rows = L * H * nq
+    rho = np.empty(rows)
+    i = 0
+    while i < rows:
+        n = int(g.integers(1, 90))
+        rho[i:i + n] = g.choice([0.0, 0.03, 0.25, 0.27, 0.6, 1.0])
+        i += n
+    bm = W.pack_bits((g.random((rows, nk)) < rho[:, None]).reshape(L, H, nq, nk))
+    bm[..., -1] |= np.uint32((0xFFFFFFFF << (nk % 32)) & 0xFFFFFFFF)
+    assert bm.size >= 1 << 20 and bm.size % 1024 != 0
+    rp, ci = check(bm, nk)
+    # capacity guard on the same path
+    rp_o, ci_o = oracle.mask_to_index(bm, nk)
+    cap = len(ci_o) - 12345
+    buf = torch.full((len(ci_o),), -7, dtype=torch.int32, device=dev())
+    B.chorus_mask_to_index(dmask(bm), nk, col_idx=buf[:cap])
+    torch.cuda.synchronize()
+    got = buf.cpu().numpy()
+    assert np.array_equal(got[:cap], ci_o[:cap]) and np.all(got[cap:] == -7)
+
+
 def test_visit_refresh_matches_oracle():
     nk, nq, H, L = 45, 3, 2, 19
     g = np.random.default_rng(3)
