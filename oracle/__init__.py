@@ -71,8 +71,11 @@ def _strides(a):
 
 
 def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_threads=0,
-                      return_weight_sum=False, return_lse=False):
+                      return_weight_sum=False, return_lse=False, n_first=0, beta=1.0):
     """fp64 block-sparse attention on the exact input bytes.
+
+    n_first, beta: first-frame key enhancement (eq. (1)): the keys of tokens
+    0 .. n_first-1 are multiplied by beta (in fp64, on the exact input values) before the scores.
 
     Q, K, V: [B][N][H][d] numpy arrays, uint16 (bf16 bits), float16, or uint8 (e4m3 codes; then
     fp8_scales = (q_scale [B][H][ceil(N/128)], k_scale same, v_scale [B][H][d]) float32).
@@ -105,7 +108,8 @@ def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_th
         _p(Q), _p(K), _p(V), C.c_int(dtype), B, H, N, d,
         *_strides(Q), *_strides(K), *_strides(V),
         _p(qs), _p(ks), _p(vs), _p(bm), C.c_double(scale),
-        n, _p(ib), _p(ih), _p(iq), _p(out), _p(ws), _p(lse), C.c_int(n_threads))
+        n, _p(ib), _p(ih), _p(iq), _p(out), _p(ws), _p(lse), C.c_int(n_threads),
+        C.c_int(int(n_first)), C.c_double(float(beta)))
     res = (out,) + ((ws,) if return_weight_sum else ()) + ((lse,) if return_lse else ())
     return res if len(res) > 1 else out
 

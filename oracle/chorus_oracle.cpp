@@ -169,7 +169,7 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
                               const uint32_t* bitmask, double scale,
                               int n_items, const int32_t* item_b, const int32_t* item_h,
                               const int32_t* item_qb, double* out, double* weight_sum,
-                              double* lse, int n_threads) {
+                              double* lse, int n_threads, int n_first, double beta) {
     (void)B;
     const int nq = (N + BQ - 1) / BQ;
     const int nk = (N + BK - 1) / BK;
@@ -209,7 +209,9 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
                 for (int c = 0; c < d; ++c) {
                     const double vs = dtype == 1 ? static_cast<double>(
                         v_scale[(static_cast<int64_t>(b) * H + h) * d + c]) : 1.0;
-                    Kd[x * d + c] = load(K, b * k_sb + j * k_sn + h * k_sh + c, ks);
+                    // first-frame key enhancement, eq. (1): K[:, 0:N0] <- beta K[:, 0:N0]
+                    const double kf = j < n_first ? beta : 1.0;
+                    Kd[x * d + c] = kf * load(K, b * k_sb + j * k_sn + h * k_sh + c, ks);
                     Vd[x * d + c] = load(V, b * v_sb + j * v_sn + h * v_sh + c, vs);
                 }
             }

@@ -268,3 +268,48 @@ def test_fp16_attention_equals_dense_numpy():
         ref = dense_softmax_attention(Q[0, :, h].astype(np.float64), K[0, :, h].astype(np.float64),
                                       V[0, :, h].astype(np.float64), scale)
         assert np.allclose(out[0, :, h], ref, rtol=1e-12, atol=1e-14)
+
+
+def test_first_frame_key_scaling_equals_dense_attention_on_scaled_keys():
+    """PAPER.md:L109-114 eq. (1): K[:, 0:N0] <- beta K[:, 0:N0], Q and V unchanged.  Pinned against numpy dense
+    attention on keys scaled by hand (N0 inside a key block, a non-representable beta), against a closed form
+    (uniform values: O unchanged; q = 0: weights unchanged), and the degenerate cases beta = 1 and N0 = 0."""
+    N, H, n0, beta = 320, 2, 100, 1.37          # n0 = 100 straddles key block 1 (64..127)
+    Q, K, V = random_qkv_bits(N, H, seed=41)
+    keep = np.ones((H, 3, 5), bool)
+    O, lse = run_oracle(Q, K, V, keep, n_first=n0, beta=beta, return_lse=True)
+    from scipy.special import logsumexp
+    for h in range(H):
+        q, k, v = (bits_to_f64(x[0, :, h]) for x in (Q, K, V))
+        k2 = k.copy()
+        k2[:n0] *= beta
+        np.testing.assert_allclose(O[0, :, h], dense_softmax_attention(q, k2, v, SCALE), rtol=0, atol=1e-12)
+        ref_lse = logsumexp((q @ k2.T) * SCALE, axis=1)
+        got = lse.reshape(H, 3, BQ)[h].reshape(-1)[:N]
+        np.testing.assert_allclose(got, ref_lse, rtol=0, atol=1e-12)
+    # beta = 1 and n_first = 0 are the plain call, bit for bit
+    plain = run_oracle(Q, K, V, keep)
+    assert np.array_equal(run_oracle(Q, K, V, keep, n_first=n0, beta=1.0), plain)
+    assert np.array_equal(run_oracle(Q, K, V, keep, n_first=0, beta=3.0), plain)
+    # it moves weight TOWARDS the first frame when the scores there are positive: with K = Q = const > 0
+    # every score is c; scaled columns get beta c: weight of the first n0 keys = n0 e^{beta c} / (...)
+    one = np.full((1, N, 1, 128), 0x3F80, np.uint16)            # bf16 1.0
+    Vb = np.zeros((1, N, 1, 128), np.uint16)
+    Vb[0, :n0] = 0x3F80                                          # V = 1 on the first frame, 0 elsewhere
+    O1 = run_oracle(one, one, Vb, np.ones((1, 3, 5), bool), scale=1.0 / 128.0, n_first=n0, beta=2.0)
+    w = n0 * np.exp(2.0) / (n0 * np.exp(2.0) + (N - n0) * np.exp(1.0))
+    np.testing.assert_allclose(O1[0, :, 0], w, rtol=1e-13)
+
+
+def test_first_frame_key_scaling_only_touches_kept_first_frame_blocks():
+    # a pruned first-frame block has no influence, scaled or not; a kept block beyond N0 is not scaled
+    N, H, n0 = 384, 1, 128
+    Q, K, V = random_qkv_bits(N, H, seed=43)
+    keep = np.zeros((H, 3, 6), bool)
+    keep[0, :, 3] = keep[0, :, 5] = True                         # only blocks beyond the first frame
+    assert np.array_equal(run_oracle(Q, K, V, keep, n_first=n0, beta=4.0), run_oracle(Q, K, V, keep))
+    keep[0, :, 1] = True                                         # one first-frame block
+    a = run_oracle(Q, K, V, keep, n_first=n0, beta=4.0)
+    K2 = K.copy()
+    K2[0, 64:128] = (bits_to_f64(K[0, 64:128]) * 4.0).astype(np.float32).view(np.uint32).__rshift__(16).astype(np.uint16)
+    np.testing.assert_allclose(a, run_oracle(Q, K2, V, keep), rtol=0, atol=1e-13)   # x4 is exact in bf16
