@@ -12,6 +12,7 @@
  *   chorus_quantize_fp8           bf16 Q/K/V -> e4m3 + scales for the FP8 backend              (L97)
  *   chorus_block_sparse_attn_fwd  block-sparse attention forward, BF16, FP16 or FP8 e4m3       (L97)
  *   chorus_block_sparse_attn_fwd_lse   the same, also writing the rows' log-sum-exp            (L87)
+ *   chorus_block_sparse_attn_fwd_first_frame   the same with first-frame key enhancement  (L109-114 eq. 1)
  * and, for the historical request whose masks get cached, and for sequence-parallel groups:
  *   chorus_block_mass / chorus_mask_from_mass / chorus_mask_coverage
  *                                 dense attention mass per block -> top-p mask with a top-k floor
@@ -156,6 +157,22 @@ chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, con
                                                const chorus_attn_shape* shape,
                                                const chorus_fp8_scales* fp8, float* lse,
                                                void* cuda_stream);
+
+/* The same call with first-frame key enhancement fused in (eq. (1):
+ * "K[:, 0:N0] <- beta_step K[:, 0:N0] ... leaving Q and V unchanged", N0 = tokens of the first
+ * frame): the scores of keys 0 .. n_first-1 are multiplied by beta inside the kernel (the scale
+ * factor of a key tile that lies in the first frame, a per-column factor in the one tile that
+ * straddles n_first), so K is neither rewritten nor re-rounded: the result is that of the plain call
+ * on keys scaled in exact arithmetic (R25).  lse, if given, is that of the scaled scores.
+ *   n_first  >= 0 (values above N act as N; 0 = no scaling);  beta  > 0 and finite.
+ * n_first == 0 or beta == 1 runs the plain kernel.  Same accuracy bounds as the plain call.
+ * Errors: as above, plus INVALID_ARG for n_first < 0 or beta not positive and finite. */
+chorus_status chorus_block_sparse_attn_fwd_first_frame(const void* Q, const void* K, const void* V,
+                                                       const int32_t* row_ptr, const int32_t* col_idx,
+                                                       float scale, chorus_dtype dtype, void* O,
+                                                       const chorus_attn_shape* shape,
+                                                       const chorus_fp8_scales* fp8, float* lse,
+                                                       int n_first, float beta, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * FP8 quantisation pre-pass for dtype = CHORUS_FP8_E4M3 (PAPER.md:L97 says only "FP8

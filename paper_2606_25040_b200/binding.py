@@ -19,7 +19,7 @@ CHORUS_BF16, CHORUS_FP8_E4M3, CHORUS_FP16 = 0, 1, 2
 BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
 
 EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
-           "chorus_block_sparse_attn_fwd_lse",
+           "chorus_block_sparse_attn_fwd_lse", "chorus_block_sparse_attn_fwd_first_frame",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
            "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count"]
@@ -73,6 +73,8 @@ def lib() -> C.CDLL:
                                                        C.c_void_p, C.c_float, C.c_int, C.c_void_p,
                                                        C.POINTER(AttnShape), C.POINTER(Fp8Scales),
                                                        C.c_void_p, C.c_void_p]
+        L.chorus_block_sparse_attn_fwd_first_frame.argtypes = (
+            L.chorus_block_sparse_attn_fwd_lse.argtypes[:-1] + [C.c_int, C.c_float, C.c_void_p])
         L.chorus_mask_from_mass.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_float, C.c_float,
                                             C.c_void_p, C.c_void_p, C.c_void_p]
         L.chorus_mask_coverage.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
@@ -165,9 +167,10 @@ def attn_shape(Q, K, V, O=None) -> AttnShape:
 
 
 def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype: int = CHORUS_BF16,
-                                 O=None, fp8_scales=None, stream=None, lse=None):
+                                 O=None, fp8_scales=None, stream=None, lse=None, n_first=0, beta=1.0):
     """Q, K, V: cuda tensors indexed [B][N][H][d] (bf16, or uint8/float8_e4m3fn codes for FP8).
-    row_ptr: this layer's H*nq+1 entries (a view into the full row_ptr is fine).  Returns O (bf16)."""
+    row_ptr: this layer's H*nq+1 entries (a view into the full row_ptr is fine).  Returns O (bf16).
+    n_first, beta: first-frame key enhancement (chorus_block_sparse_attn_fwd_first_frame)."""
     assert Q.is_cuda and K.is_cuda and V.is_cuda
     B, N, H, d = Q.shape
     if Q.dtype == torch.float16:          # the paper's non-quantised path (PAPER.md:L97): fp16 in, fp16 out
@@ -181,6 +184,14 @@ def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype:
         sc = Fp8Scales(*(x.data_ptr() for x in fp8_scales))
     if lse is not None:     # float32 [B][H][N], written by the kernel (natural-log row log-sum-exp)
         assert lse.dtype == torch.float32 and lse.is_contiguous() and lse.shape == (B, H, N)
+    if n_first != 0 or beta != 1.0:
+        _check(lib().chorus_block_sparse_attn_fwd_first_frame(
+            _ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx), C.c_float(scale), dtype, _ptr(O),
+            C.byref(shape), C.byref(sc) if sc is not None else None,
+            _ptr(lse) if lse is not None else None, C.c_int(int(n_first)), C.c_float(float(beta)),
+            _stream(stream)))
+        return O
+    if lse is not None:
         _check(lib().chorus_block_sparse_attn_fwd_lse(_ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx),
                                                       C.c_float(scale), dtype, _ptr(O), C.byref(shape),
                                                       C.byref(sc) if sc is not None else None,

@@ -154,7 +154,8 @@ __device__ __forceinline__ float max64(const uint32_t* sv) {
     return fmaxf(fmaxf(a0, a1), fmaxf(a2, a3));
 }
 
-template <bool kFp8, bool kF16>   // e4m3 inputs / fp16 inputs and output (neither: bf16)
+// kBeta: first-frame key enhancement (eq. (1)) as a factor on the scores of keys < n_first
+template <bool kFp8, bool kF16, bool kBeta>   // e4m3 inputs / fp16 inputs and output (neither: bf16)
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmO,
@@ -371,6 +372,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const int64_t sbase = (static_cast<int64_t>(it.b) * p.H + it.h) * nsb;
                 qsl2 = p.scale_log2 * __ldg(p.q_scale + sbase + it.qb);
                 ksc = p.k_scale + sbase;
+            }
+            if constexpr (kFp8 || kBeta) {
                 if (2 * sm < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * sm);
                 if (2 * sm + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * sm + 1);
             }
@@ -379,16 +382,28 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const uint32_t tS = tlane + TM_S + sb * 128;     // this pair's S, overwritten by its P
                 int va = BK, vb = BK;            // valid keys in the two tiles of the pair
                 int kba = 0, kbb = 0;
-                if constexpr (kFp8) {
+                if constexpr (kFp8 || kBeta) {
                     kba = kba_next;
                     kbb = kbb_next;
                     if (2 * (j + 2) < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2));
                     if (2 * (j + 2) + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2) + 1);
+                }
+                if constexpr (kFp8) {
                     sl2a = qsl2 * __ldg(ksc + (kba >> 1));
                     sl2b = qsl2 * __ldg(ksc + (kbb >> 1));
                 }
+                // kBeta: a tile inside the first frame takes beta in its scale factor; the one tile
+                // that straddles n_first takes it per column (fa / fb leading columns) in the masked body
+                int fa = 0, fb = 0;
+                if constexpr (kBeta) {
+                    if constexpr (!kFp8) sl2a = sl2b = p.scale_log2;
+                    fa = min(BK, max(0, p.n_first - kba * BK));
+                    fb = (2 * j + 1 < it.nt) ? min(BK, max(0, p.n_first - kbb * BK)) : 0;
+                    if (fa == BK) { sl2a *= p.beta; fa = 0; }
+                    if (fb == BK) { sl2b *= p.beta; fb = 0; }
+                }
                 if (j == it.np - 1) {            // only the last pair can be odd or hold the ragged key block
-                    if constexpr (!kFp8) {
+                    if constexpr (!(kFp8 || kBeta)) {
                         kba = __ldg(p.col_idx + it.r0 + 2 * j);
                         if (2 * j + 1 < it.nt) kbb = __ldg(p.col_idx + it.r0 + 2 * j + 1);
                     }
@@ -402,7 +417,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 // The 128 scores of a row are streamed from tensor memory twice, 32 columns at a time
                 // with the next chunk's load in flight (pass 1: row max; pass 2: exp, pack, store P
                 // behind the read position), so that only 64 of them are ever live in registers.
-                const bool ragged = (va < BK) || (vb < BK);   // warp-uniform, last pair of a row only
+                const bool ragged = (va < BK) || (vb < BK) || (fa | fb) != 0;   // warp-uniform and rare
                 // The body is instantiated twice (with / without tail masking) so that the common
                 // case carries no branch: the compiler can then schedule across the chunks.
                 auto pair_body = [&](auto rag_tag) {
@@ -412,6 +427,12 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
                     for (int k = 0; k < 32; ++k)
                         if (k >= valid) r[k] = 0xff800000u;   // -inf
+                    if constexpr (kBeta) {
+                        const int nf = ((c >> 1) ? fb : fa) - 32 * (c & 1);
+#pragma unroll
+                        for (int k = 0; k < 32; ++k)
+                            if (k < nf) r[k] = __float_as_uint(__uint_as_float(r[k]) * p.beta);
+                    }
                 };
                 auto max32 = [](const uint32_t (&r)[32]) {
                     float a0 = -INFINITY, a1 = -INFINITY;
@@ -662,18 +683,18 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 }  // namespace
 
-template <bool kFp8, bool kF16>
+template <bool kFp8, bool kF16, bool kBeta>
 static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                               const CUtensorMap& tmO, const AttnParams& p, cudaStream_t stream) {
     constexpr uint32_t smem = Cfg<kFp8>::SMEM_BYTES;
-    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kFp8, kF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kFp8, kF16, kBeta>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     const int n_items = p.B * p.H * p.nq;
     const int grid = n_items < sms ? n_items : sms;
-    attn_fwd_kernel<kFp8, kF16><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
+    attn_fwd_kernel<kFp8, kF16, kBeta><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
     count_launch(1);
     return cudaGetLastError();
 }
@@ -681,9 +702,15 @@ static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, co
 cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
                             cudaStream_t stream) {
-    if (dtype == CHORUS_BF16) return launch_one<false, false>(tmQ, tmK, tmV, tmO, p, stream);
-    if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false>(tmQ, tmK, tmV, tmO, p, stream);
-    if (dtype == CHORUS_FP16) return launch_one<false, true>(tmQ, tmK, tmV, tmO, p, stream);
+    if (p.n_first > 0 && p.beta != 1.f) {
+        if (dtype == CHORUS_BF16) return launch_one<false, false, true>(tmQ, tmK, tmV, tmO, p, stream);
+        if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, true>(tmQ, tmK, tmV, tmO, p, stream);
+        if (dtype == CHORUS_FP16) return launch_one<false, true, true>(tmQ, tmK, tmV, tmO, p, stream);
+        return cudaErrorNotSupported;
+    }
+    if (dtype == CHORUS_BF16) return launch_one<false, false, false>(tmQ, tmK, tmV, tmO, p, stream);
+    if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, false>(tmQ, tmK, tmV, tmO, p, stream);
+    if (dtype == CHORUS_FP16) return launch_one<false, true, false>(tmQ, tmK, tmV, tmO, p, stream);
     return cudaErrorNotSupported;
 }
 

@@ -180,7 +180,20 @@ chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, con
                                                const chorus_attn_shape* shape,
                                                const chorus_fp8_scales* fp8, float* lse,
                                                void* cuda_stream) {
+    return chorus_block_sparse_attn_fwd_first_frame(Q, K, V, row_ptr, col_idx, scale, dtype, O, shape, fp8,
+                                                    lse, 0, 1.0f, cuda_stream);
+}
+
+chorus_status chorus_block_sparse_attn_fwd_first_frame(const void* Q, const void* K, const void* V,
+                                                       const int32_t* row_ptr, const int32_t* col_idx,
+                                                       float scale, chorus_dtype dtype, void* O,
+                                                       const chorus_attn_shape* shape,
+                                                       const chorus_fp8_scales* fp8, float* lse,
+                                                       int n_first, float beta, void* cuda_stream) {
     g_err[0] = 0;
+    if (n_first < 0) return set_error(CHORUS_ERR_INVALID_ARG, "n_first = %d is negative", n_first);
+    if (!(beta > 0.f) || !(beta <= 3.0e38f))
+        return set_error(CHORUS_ERR_INVALID_ARG, "beta = %g must be positive and finite", static_cast<double>(beta));
     if (dtype != CHORUS_BF16 && dtype != CHORUS_FP8_E4M3 && dtype != CHORUS_FP16)
         return set_error(CHORUS_ERR_UNSUPPORTED, "unknown dtype %d", static_cast<int>(dtype));
     if (!Q || !K || !V || !O || !row_ptr || !col_idx)
@@ -220,6 +233,8 @@ chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, con
     p.k_scale = fp8 ? fp8->k_scale : nullptr;
     p.v_scale = fp8 ? fp8->v_scale : nullptr;
     p.lse = lse;
+    p.n_first = n_first < s.N ? n_first : s.N;
+    p.beta = beta;
     cudaError_t e = launch_attn_fwd(tmQ, tmK, tmV, tmO, p, dtype, static_cast<cudaStream_t>(cuda_stream));
     if (e == cudaErrorNotSupported)
         return set_error(CHORUS_ERR_UNSUPPORTED, "dtype %d not implemented by this build", (int)dtype);

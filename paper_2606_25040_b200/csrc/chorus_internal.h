@@ -45,6 +45,8 @@ struct AttnParams {
     const float* k_scale;
     const float* v_scale;
     float* lse;  // optional [B][H][N] row log-sum-exp (natural log), or null
+    int n_first;  // first-frame key enhancement (eq. 1): scores of keys < n_first are multiplied by beta
+    float beta;   // > 0; n_first = 0 or beta = 1 selects the plain kernel
 };
 cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
