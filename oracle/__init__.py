@@ -25,6 +25,7 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(_build())
         _lib.oracle_mask_to_index.restype = C.c_int64
+        _lib.oracle_mask_to_index_64x128.restype = C.c_int64
         _lib.oracle_e4m3_to_double.restype = C.c_double
         _lib.oracle_e4m3_to_double.argtypes = [C.c_uint8]
         _lib.oracle_f16_to_double.restype = C.c_double
@@ -62,6 +63,20 @@ def mask_to_index(bitmask: np.ndarray, nk: int, count_only: bool = False):
     return row_ptr, col_idx[:nnz]
 
 
+def mask_to_index_64x128(bitmask: np.ndarray, N: int):
+    """Paper geometry (64 query rows x 128 keys): bitmask uint32 [L][H][ceil(N/64)][words] ->
+    (row_ptr int32 [L*H*ceil(N/128)+1], col_idx uint32: 64-key tile | bit 30 = rows 0-63 of the 128-row block do
+    not keep it | bit 31 = rows 64-127 do not keep it)."""
+    bm = _c(bitmask, np.uint32)
+    L, H, nq64, words = bm.shape
+    assert nq64 == (N + 63) // 64 and words == ((N + 127) // 128 + 31) // 32
+    row_ptr = np.zeros(L * H * ((N + 127) // 128) + 1, dtype=np.int32)
+    nnz = lib().oracle_mask_to_index_64x128(_p(bm), L, H, N, _p(row_ptr), None)
+    col_idx = np.zeros(max(int(nnz), 1), dtype=np.uint32)
+    lib().oracle_mask_to_index_64x128(_p(bm), L, H, N, _p(row_ptr), _p(col_idx))
+    return row_ptr, col_idx[:nnz]
+
+
 def _strides(a):
     # element strides of a [B][N][H][d] array whose last dim is contiguous
     es = a.dtype.itemsize
@@ -71,9 +86,11 @@ def _strides(a):
 
 
 def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_threads=0,
-                      return_weight_sum=False, return_lse=False, n_first=0, beta=1.0):
+                      return_weight_sum=False, return_lse=False, n_first=0, beta=1.0, block=(128, 64)):
     """fp64 block-sparse attention on the exact input bytes.
 
+    block = (query rows, keys) per mask block: (128, 64) or the paper's (64, 128); items, the
+    bitmask's shape and the output rows follow it.
     n_first, beta: first-frame key enhancement (eq. (1)): the keys of tokens
     0 .. n_first-1 are multiplied by beta (in fp64, on the exact input values) before the scores.
 
@@ -86,6 +103,8 @@ def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_th
     assert Q.dtype == K.dtype == V.dtype and Q.dtype in (np.uint16, np.uint8, np.float16)
     dtype = {np.dtype(np.uint16): 0, np.dtype(np.uint8): 1, np.dtype(np.float16): 2}[Q.dtype]
     B, N, H, d = Q.shape
+    BQ, BK = block
+    assert (BQ, BK) in ((128, 64), (64, 128))
     nq, nk = (N + BQ - 1) // BQ, (N + BK - 1) // BK
     bm = _c(bitmask, np.uint32)
     assert bm.shape == (H, nq, (nk + 31) // 32), (bm.shape, (H, nq, (nk + 31) // 32))
@@ -109,7 +128,7 @@ def block_sparse_attn(Q, K, V, bitmask, scale, items=None, fp8_scales=None, n_th
         *_strides(Q), *_strides(K), *_strides(V),
         _p(qs), _p(ks), _p(vs), _p(bm), C.c_double(scale),
         n, _p(ib), _p(ih), _p(iq), _p(out), _p(ws), _p(lse), C.c_int(n_threads),
-        C.c_int(int(n_first)), C.c_double(float(beta)))
+        C.c_int(int(n_first)), C.c_double(float(beta)), C.c_int(BQ), C.c_int(BK))
     res = (out,) + ((ws,) if return_weight_sum else ()) + ((lse,) if return_lse else ())
     return res if len(res) > 1 else out
 

@@ -141,6 +141,42 @@ int64_t oracle_mask_to_index(const uint32_t* bitmask, int L, int H, int nq, int 
 }
 
 // -------------------------------------------------------------------------------------------------
+// f-4  Decode of a mask in the paper's own geometry (64 query rows x 128 keys per
+// block) into the index the 128 x 64 kernel walks (R26).  bitmask is
+// [L][H][nq64][words], nq64 = ceil(N/64), bit kb of a row = key block kb (keys 128 kb .. 128 kb + 127)
+// of nk128 = ceil(N/128).  Output row R = (l, h, qb128) covers mask rows 2 qb128 ("upper", query
+// rows 0-63 of the 128) and 2 qb128 + 1 ("lower", if it exists).  For every key block kept by
+// EITHER of them, ascending, and for each of its two 64-key tiles t = 2 kb, 2 kb + 1 with
+// 64 t < N, one entry:  t | (upper does not keep kb) << 30 | (lower does not keep kb) << 31.
+// Returns the number of entries; col_idx may be null (count only).
+// -------------------------------------------------------------------------------------------------
+int64_t oracle_mask_to_index_64x128(const uint32_t* bitmask, int L, int H, int N,
+                                    int32_t* row_ptr, uint32_t* col_idx) {
+    const int nq64 = (N + 63) / 64, nk128 = (N + 127) / 128, nq128 = (N + 127) / 128;
+    const int words = (nk128 + 31) / 32;
+    int64_t nnz = 0, R = 0;
+    row_ptr[0] = 0;
+    for (int l = 0; l < L; ++l)
+        for (int h = 0; h < H; ++h)
+            for (int qb = 0; qb < nq128; ++qb, ++R) {
+                const uint32_t* up = bitmask + ((static_cast<int64_t>(l) * H + h) * nq64 + 2 * qb) * words;
+                const uint32_t* lo = (2 * qb + 1 < nq64) ? up + words : nullptr;
+                for (int kb = 0; kb < nk128; ++kb) {
+                    const bool ku = mask_bit(up, kb), kl = lo != nullptr && mask_bit(lo, kb);
+                    if (!ku && !kl) continue;
+                    for (int t = 2 * kb; t <= 2 * kb + 1; ++t) {
+                        if (64 * t >= N) continue;
+                        if (col_idx)
+                            col_idx[nnz] = static_cast<uint32_t>(t) | (ku ? 0u : 1u << 30) | (kl ? 0u : 1u << 31);
+                        ++nnz;
+                    }
+                }
+                row_ptr[R + 1] = static_cast<int32_t>(nnz);
+            }
+    return nnz;
+}
+
+// -------------------------------------------------------------------------------------------------
 // a-2 / a-3  Block-sparse attention.  PAPER.md:L97: "skip pruned block pairs and
 // evaluate only the retained ones in QK^T, softmax, and PV" => the softmax is normalised over the
 // retained keys only (R5).  For head h and query i (qb = i / 128):
@@ -169,8 +205,11 @@ void oracle_block_sparse_attn(const void* Q, const void* K, const void* V, int d
                               const uint32_t* bitmask, double scale,
                               int n_items, const int32_t* item_b, const int32_t* item_h,
                               const int32_t* item_qb, double* out, double* weight_sum,
-                              double* lse, int n_threads, int n_first, double beta) {
+                              double* lse, int n_threads, int n_first, double beta, int bq, int bk) {
     (void)B;
+    // block geometry: 128 x 64 (BASELINE.json north_star) unless the caller asks for the paper's own
+    // 64 x 128; it only decides which keys a query row retains
+    const int BQ = bq > 0 ? bq : ::BQ, BK = bk > 0 ? bk : ::BK;
     const int nq = (N + BQ - 1) / BQ;
     const int nk = (N + BK - 1) / BK;
     const int words = (nk + 31) / 32;
