@@ -13,6 +13,8 @@
  *   chorus_block_sparse_attn_fwd  block-sparse attention forward, BF16, FP16 or FP8 e4m3       (L97)
  *   chorus_block_sparse_attn_fwd_lse   the same, also writing the rows' log-sum-exp            (L87)
  *   chorus_block_sparse_attn_fwd_first_frame   the same with first-frame key enhancement  (L109-114 eq. 1)
+ *   chorus_mask_to_index_64x128 / chorus_block_sparse_attn_fwd_64x128
+ *                                 the same path for masks in the paper's own 64 x 128 block geometry (L153)
  * and, for the historical request whose masks get cached, and for sequence-parallel groups:
  *   chorus_block_mass / chorus_mask_from_mass / chorus_mask_coverage
  *                                 dense attention mass per block -> top-p mask with a top-k floor
@@ -173,6 +175,40 @@ chorus_status chorus_block_sparse_attn_fwd_first_frame(const void* Q, const void
                                                        const chorus_attn_shape* shape,
                                                        const chorus_fp8_scales* fp8, float* lse,
                                                        int n_first, float beta, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Masks in the paper's own block geometry ("block size for sparse attention 64 x 128":
+ * 64 query rows x 128 keys per mask block; R26).  The kernel keeps its 128 x 64 tiles:
+ *
+ * chorus_mask_to_index_64x128
+ *   bitmask   device, uint32 [L][H][ceil(N/64)][words], words = ceil(ceil(N/128) / 32); bit kb of a
+ *             row = key block kb (keys 128 kb .. 128 kb + 127); pad bits are ignored.
+ *   row_ptr   device, int32 [L*H*ceil(N/128) + 1]: row (l, h, qb) covers mask rows 2 qb ("upper":
+ *             query rows 0-63 of the 128) and 2 qb + 1 ("lower", if it exists).
+ *   col_idx   device, int32 [col_cap] or NULL (count only).  For every key block kept by EITHER mask
+ *             row, ascending, and each of its two 64-key tiles t = 2 kb, 2 kb + 1 with 64 t < N, one
+ *             entry  t | (upper does not keep kb) << 30 | (lower does not keep kb) << 31.
+ *             An entry without flag bits is a plain chorus_mask_to_index entry.
+ *   workspace as for chorus_mask_to_index (NULL = size query), 16-byte aligned.
+ *   Unique result, compared bit-exactly with the oracle.  Three launches (tile mask of the row pairs,
+ *   the plain decode, the flags).
+ *
+ * chorus_block_sparse_attn_fwd_64x128
+ *   The attention call (arguments as chorus_block_sparse_attn_fwd_lse) on such an index: query row i
+ *   attends the keys of the key blocks its own 64-row mask row keeps, exactly; the tiles a 128-row
+ *   block's other half alone keeps are computed and masked (up to 2x the tile work of the mask when
+ *   the two halves share nothing, none when they agree).  Same accuracy bounds as the plain call.
+ * Errors: as the plain calls.
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_mask_to_index_64x128(const uint32_t* bitmask, int L, int H, int N,
+                                          int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
+                                          void* workspace, size_t* workspace_bytes, void* cuda_stream);
+chorus_status chorus_block_sparse_attn_fwd_64x128(const void* Q, const void* K, const void* V,
+                                                  const int32_t* row_ptr, const int32_t* col_idx,
+                                                  float scale, chorus_dtype dtype, void* O,
+                                                  const chorus_attn_shape* shape,
+                                                  const chorus_fp8_scales* fp8, float* lse,
+                                                  void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * FP8 quantisation pre-pass for dtype = CHORUS_FP8_E4M3 (PAPER.md:L97 says only "FP8

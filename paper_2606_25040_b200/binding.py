@@ -20,6 +20,7 @@ BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
 
 EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
            "chorus_block_sparse_attn_fwd_lse", "chorus_block_sparse_attn_fwd_first_frame",
+           "chorus_mask_to_index_64x128", "chorus_block_sparse_attn_fwd_64x128",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
            "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count"]
@@ -75,6 +76,9 @@ def lib() -> C.CDLL:
                                                        C.c_void_p, C.c_void_p]
         L.chorus_block_sparse_attn_fwd_first_frame.argtypes = (
             L.chorus_block_sparse_attn_fwd_lse.argtypes[:-1] + [C.c_int, C.c_float, C.c_void_p])
+        L.chorus_block_sparse_attn_fwd_64x128.argtypes = L.chorus_block_sparse_attn_fwd_lse.argtypes
+        L.chorus_mask_to_index_64x128.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                                  C.c_int64, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p]
         L.chorus_mask_from_mass.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_float, C.c_float,
                                             C.c_void_p, C.c_void_p, C.c_void_p]
         L.chorus_mask_coverage.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
@@ -146,6 +150,33 @@ def chorus_mask_to_index(bitmask, nk_blk: int, row_ptr=None, col_idx=None, works
     return row_ptr, col_idx
 
 
+def chorus_mask_to_index_64x128(bitmask, N: int, row_ptr=None, col_idx=None, workspace=None, stream=None,
+                                count_only=False):
+    """bitmask: cuda 4-byte tensor [L][H][ceil(N/64)][words] in the paper's 64 x 128 geometry.  Returns
+    (row_ptr [L*H*ceil(N/128)+1], col_idx with the per-half flag bits) for chorus_block_sparse_attn_fwd(...,
+    geometry_64x128=True).  Same two-pass protocol as chorus_mask_to_index."""
+    L, H, nq64, words = bitmask.shape
+    assert bitmask.is_cuda and bitmask.is_contiguous() and bitmask.element_size() == 4
+    assert nq64 == (N + 63) // 64 and words == ((N + 127) // 128 + 31) // 32
+    dev = bitmask.device
+    if row_ptr is None:
+        row_ptr = torch.empty(L * H * ((N + 127) // 128) + 1, dtype=torch.int32, device=dev)
+    if workspace is None:
+        need = C.c_size_t(0)
+        _check(lib().chorus_mask_to_index_64x128(None, L, H, N, None, None, 0, None, C.byref(need), None))
+        workspace = torch.empty(max(need.value, 16), dtype=torch.uint8, device=dev)
+    wsb = C.c_size_t(workspace.numel())
+    if col_idx is None:
+        _check(lib().chorus_mask_to_index_64x128(_ptr(bitmask), L, H, N, _ptr(row_ptr), None, 0,
+                                                 _ptr(workspace), C.byref(wsb), _stream(stream)))
+        if count_only:
+            return row_ptr, None
+        col_idx = torch.empty(max(int(row_ptr[-1].item()), 1), dtype=torch.int32, device=dev)
+    _check(lib().chorus_mask_to_index_64x128(_ptr(bitmask), L, H, N, _ptr(row_ptr), _ptr(col_idx),
+                                             col_idx.numel(), _ptr(workspace), C.byref(wsb), _stream(stream)))
+    return row_ptr, col_idx
+
+
 def chorus_visit_refresh(bitmask, nk_blk: int, group: int = 8, stream=None):
     L, H, nq, words = bitmask.shape
     assert bitmask.is_cuda and bitmask.is_contiguous() and bitmask.element_size() == 4
@@ -167,10 +198,12 @@ def attn_shape(Q, K, V, O=None) -> AttnShape:
 
 
 def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype: int = CHORUS_BF16,
-                                 O=None, fp8_scales=None, stream=None, lse=None, n_first=0, beta=1.0):
+                                 O=None, fp8_scales=None, stream=None, lse=None, n_first=0, beta=1.0,
+                                 geometry_64x128=False):
     """Q, K, V: cuda tensors indexed [B][N][H][d] (bf16, or uint8/float8_e4m3fn codes for FP8).
     row_ptr: this layer's H*nq+1 entries (a view into the full row_ptr is fine).  Returns O (bf16).
-    n_first, beta: first-frame key enhancement (chorus_block_sparse_attn_fwd_first_frame)."""
+    n_first, beta: first-frame key enhancement (chorus_block_sparse_attn_fwd_first_frame).
+    geometry_64x128: row_ptr / col_idx come from chorus_mask_to_index_64x128 (chorus_block_sparse_attn_fwd_64x128)."""
     assert Q.is_cuda and K.is_cuda and V.is_cuda
     B, N, H, d = Q.shape
     if Q.dtype == torch.float16:          # the paper's non-quantised path (PAPER.md:L97): fp16 in, fp16 out
@@ -184,6 +217,14 @@ def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype:
         sc = Fp8Scales(*(x.data_ptr() for x in fp8_scales))
     if lse is not None:     # float32 [B][H][N], written by the kernel (natural-log row log-sum-exp)
         assert lse.dtype == torch.float32 and lse.is_contiguous() and lse.shape == (B, H, N)
+    if geometry_64x128:
+        if n_first != 0 or beta != 1.0:
+            raise ChorusError(2, "first-frame scaling and the 64 x 128 geometry are not built together")
+        _check(lib().chorus_block_sparse_attn_fwd_64x128(
+            _ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx), C.c_float(scale), dtype, _ptr(O),
+            C.byref(shape), C.byref(sc) if sc is not None else None,
+            _ptr(lse) if lse is not None else None, _stream(stream)))
+        return O
     if n_first != 0 or beta != 1.0:
         _check(lib().chorus_block_sparse_attn_fwd_first_frame(
             _ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx), C.c_float(scale), dtype, _ptr(O),

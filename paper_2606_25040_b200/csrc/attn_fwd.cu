@@ -155,7 +155,9 @@ __device__ __forceinline__ float max64(const uint32_t* sv) {
 }
 
 // kBeta: first-frame key enhancement (eq. (1)) as a factor on the scores of keys < n_first
-template <bool kFp8, bool kF16, bool kBeta>   // e4m3 inputs / fp16 inputs and output (neither: bf16)
+// kHalf: col_idx entries carry per-half flags (bit 30 / 31: query rows 0-63 / 64-127 of the block do NOT keep the
+// tile), as chorus_mask_to_index_64x128 writes them for masks in the paper's 64 x 128 geometry
+template <bool kFp8, bool kF16, bool kBeta, bool kHalf>   // e4m3 inputs / fp16 inputs and output (neither: bf16)
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmO,
@@ -228,7 +230,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 // the key-block indices of 16 pairs are fetched with one coalesced load
                 for (int j0 = 0; j0 < it.np; j0 += 16) {
                     const int t = 2 * j0 + lane;
-                    const int mine = (t < it.nt) ? __ldg(p.col_idx + it.r0 + t) : 0;
+                    int mine = (t < it.nt) ? __ldg(p.col_idx + it.r0 + t) : 0;
+                    if constexpr (kHalf) mine &= 0x3fffffff;
                     const int jn = min(16, it.np - j0);
                     for (int jl = 0; jl < jn; ++jl, ++g) {
                         const int ntile = (2 * (j0 + jl) + 1 < it.nt) ? 2 : 1;
@@ -373,7 +376,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 qsl2 = p.scale_log2 * __ldg(p.q_scale + sbase + it.qb);
                 ksc = p.k_scale + sbase;
             }
-            if constexpr (kFp8 || kBeta) {
+            if constexpr (kFp8 || kBeta || kHalf) {
                 if (2 * sm < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * sm);
                 if (2 * sm + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * sm + 1);
             }
@@ -382,11 +385,19 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const uint32_t tS = tlane + TM_S + sb * 128;     // this pair's S, overwritten by its P
                 int va = BK, vb = BK;            // valid keys in the two tiles of the pair
                 int kba = 0, kbb = 0;
-                if constexpr (kFp8 || kBeta) {
+                if constexpr (kFp8 || kBeta || kHalf) {
                     kba = kba_next;
                     kbb = kbb_next;
                     if (2 * (j + 2) < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2));
                     if (2 * (j + 2) + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2) + 1);
+                }
+                uint32_t skip_a = 0u, skip_b = 0u;   // kHalf: this warp's rows do not keep tile a / b
+                if constexpr (kHalf) {
+                    const int hb = 30 + (wq >> 1);
+                    skip_a = (static_cast<uint32_t>(kba) >> hb) & 1u;
+                    skip_b = (static_cast<uint32_t>(kbb) >> hb) & 1u;
+                    kba &= 0x3fffffff;
+                    kbb &= 0x3fffffff;
                 }
                 if constexpr (kFp8) {
                     sl2a = qsl2 * __ldg(ksc + (kba >> 1));
@@ -403,12 +414,16 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     if (fb == BK) { sl2b *= p.beta; fb = 0; }
                 }
                 if (j == it.np - 1) {            // only the last pair can be odd or hold the ragged key block
-                    if constexpr (!(kFp8 || kBeta)) {
+                    if constexpr (!(kFp8 || kBeta || kHalf)) {
                         kba = __ldg(p.col_idx + it.r0 + 2 * j);
                         if (2 * j + 1 < it.nt) kbb = __ldg(p.col_idx + it.r0 + 2 * j + 1);
                     }
                     va = min(BK, p.N - kba * BK);
                     vb = (2 * j + 1 < it.nt) ? min(BK, p.N - kbb * BK) : 0;
+                }
+                if constexpr (kHalf) {           // a tile the rows of this warp do not keep: all -inf
+                    if (skip_a) va = 0;
+                    if (skip_b) vb = 0;
                 }
                 PHASE_MARK(0);
                 mbar_wait(bar(C::B_S_FULL + sb), (g / SBUFS) & 1);
@@ -514,7 +529,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     // P = exp2(s * sl2 - m_ref + shift).  Element pairs go through packed FFMA2; the
                     // pairs whose bit is set in POLY_MASK (index mod 8) take the polynomial exp2 on
                     // the FMA pipe, the rest the MUFU.
-                    const float2 negm_2 = make_float2(C::P_SHIFT - m_ref, C::P_SHIFT - m_ref);
+                    // kHalf: a row that has kept nothing so far has m_ref = -inf and only -inf scores
+                    const float negm = (kHalf && m_ref == -INFINITY) ? 0.f : C::P_SHIFT - m_ref;
+                    const float2 negm_2 = make_float2(negm, negm);
                     const float2 sl2a_2 = make_float2(sl2a, sl2a), sl2b_2 = make_float2(sl2b, sl2b);
                     float2 lacc = make_float2(l0, l1);
                     // 32 scores -> 16 (bf16) / 8 (e4m3) TMEM columns of P at chunk position c
@@ -575,7 +592,31 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 if (j + 1 < it.np) named_bar_arrive(NB_HAND + sm * 4 + wq, 64);
 #endif
                 };
-                if (ragged) pair_body(BoolTag<true>{});
+                // kHalf: the rows of this warp keep neither tile of the pair (the other half of the block
+                // does): no pass over S, P = 0, the reference is handed on unchanged
+                auto skip_body = [&]() {
+                    if (j > 0) {
+                        named_bar_sync(NB_HAND + (sm ^ 1) * 4 + wq, 64);
+                        const float m_in = xm[row];
+                        if (m_in != m_ref) {
+                            const float a = ex2(m_ref - m_in);
+                            l0 *= a;
+                            l1 *= a;
+                            m_ref = m_in;
+                        }
+                    }
+                    if (j + 1 < it.np) {
+                        xm[row] = m_ref;
+                        named_bar_arrive(NB_HAND + sm * 4 + wq, 64);
+                    }
+                    uint32_t z[16];
+#pragma unroll
+                    for (int k = 0; k < 16; ++k) z[k] = 0u;
+#pragma unroll
+                    for (int c = 0; c < (kFp8 ? 2 : 4); ++c) tmem_st16(tS + c * 16, z);
+                };
+                if (kHalf && va == 0 && vb == 0) skip_body();
+                else if (ragged) pair_body(BoolTag<true>{});
                 else pair_body(BoolTag<false>{});
                 PHASE_MARK(4);
                 tc_wait_st();
@@ -683,18 +724,18 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 }  // namespace
 
-template <bool kFp8, bool kF16, bool kBeta>
+template <bool kFp8, bool kF16, bool kBeta, bool kHalf>
 static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                               const CUtensorMap& tmO, const AttnParams& p, cudaStream_t stream) {
     constexpr uint32_t smem = Cfg<kFp8>::SMEM_BYTES;
-    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kFp8, kF16, kBeta>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kFp8, kF16, kBeta, kHalf>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     const int n_items = p.B * p.H * p.nq;
     const int grid = n_items < sms ? n_items : sms;
-    attn_fwd_kernel<kFp8, kF16, kBeta><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
+    attn_fwd_kernel<kFp8, kF16, kBeta, kHalf><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
     count_launch(1);
     return cudaGetLastError();
 }
@@ -702,15 +743,23 @@ static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, co
 cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
                             cudaStream_t stream) {
-    if (p.n_first > 0 && p.beta != 1.f) {
-        if (dtype == CHORUS_BF16) return launch_one<false, false, true>(tmQ, tmK, tmV, tmO, p, stream);
-        if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, true>(tmQ, tmK, tmV, tmO, p, stream);
-        if (dtype == CHORUS_FP16) return launch_one<false, true, true>(tmQ, tmK, tmV, tmO, p, stream);
+    const bool beta = p.n_first > 0 && p.beta != 1.f;
+    if (beta && p.half_flags) return cudaErrorNotSupported;   // not instantiated together
+    if (p.half_flags) {
+        if (dtype == CHORUS_BF16) return launch_one<false, false, false, true>(tmQ, tmK, tmV, tmO, p, stream);
+        if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, false, true>(tmQ, tmK, tmV, tmO, p, stream);
+        if (dtype == CHORUS_FP16) return launch_one<false, true, false, true>(tmQ, tmK, tmV, tmO, p, stream);
         return cudaErrorNotSupported;
     }
-    if (dtype == CHORUS_BF16) return launch_one<false, false, false>(tmQ, tmK, tmV, tmO, p, stream);
-    if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, false>(tmQ, tmK, tmV, tmO, p, stream);
-    if (dtype == CHORUS_FP16) return launch_one<false, true, false>(tmQ, tmK, tmV, tmO, p, stream);
+    if (beta) {
+        if (dtype == CHORUS_BF16) return launch_one<false, false, true, false>(tmQ, tmK, tmV, tmO, p, stream);
+        if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, true, false>(tmQ, tmK, tmV, tmO, p, stream);
+        if (dtype == CHORUS_FP16) return launch_one<false, true, true, false>(tmQ, tmK, tmV, tmO, p, stream);
+        return cudaErrorNotSupported;
+    }
+    if (dtype == CHORUS_BF16) return launch_one<false, false, false, false>(tmQ, tmK, tmV, tmO, p, stream);
+    if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, false, false>(tmQ, tmK, tmV, tmO, p, stream);
+    if (dtype == CHORUS_FP16) return launch_one<false, true, false, false>(tmQ, tmK, tmV, tmO, p, stream);
     return cudaErrorNotSupported;
 }
 

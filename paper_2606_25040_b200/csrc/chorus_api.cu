@@ -123,6 +123,37 @@ chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq
                       "mask decode launch");
 }
 
+chorus_status chorus_mask_to_index_64x128(const uint32_t* bitmask, int L, int H, int N,
+                                          int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
+                                          void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!workspace_bytes) return set_error(CHORUS_ERR_INVALID_ARG, "workspace_bytes is null");
+    if (L <= 0 || H <= 0 || N <= 0)
+        return set_error(CHORUS_ERR_INVALID_ARG, "L, H, N must be positive (%d %d %d)", L, H, N);
+    const int64_t heads = static_cast<int64_t>(L) * H;
+    const int64_t nq128 = (static_cast<int64_t>(N) + 127) / 128, nk64 = (static_cast<int64_t>(N) + 63) / 64;
+    if (heads * nq128 * nk64 > INT32_MAX)
+        return set_error(CHORUS_ERR_CAPACITY, "L*H*ceil(N/128)*ceil(N/64) = %lld exceeds INT32_MAX",
+                         static_cast<long long>(heads * nq128 * nk64));
+    const size_t need = decode_64x128_workspace_bytes(heads, N);
+    if (!workspace) {
+        *workspace_bytes = need;
+        return CHORUS_OK;
+    }
+    if (!bitmask || !row_ptr) return set_error(CHORUS_ERR_INVALID_ARG, "bitmask / row_ptr is null");
+    if (col_cap < 0) return set_error(CHORUS_ERR_INVALID_ARG, "col_cap < 0");
+    if ((reinterpret_cast<uintptr_t>(bitmask) | reinterpret_cast<uintptr_t>(row_ptr) |
+         reinterpret_cast<uintptr_t>(col_idx)) & 3u)
+        return set_error(CHORUS_ERR_INVALID_ARG, "pointers must be 4-byte aligned");
+    if (reinterpret_cast<uintptr_t>(workspace) & 15u)
+        return set_error(CHORUS_ERR_INVALID_ARG, "workspace must be 16-byte aligned");
+    if (*workspace_bytes < need)
+        return set_error(CHORUS_ERR_CAPACITY, "workspace too small: %zu < %zu", *workspace_bytes, need);
+    return check_cuda(launch_mask_decode_64x128(bitmask, heads, N, row_ptr, col_idx, col_cap, workspace,
+                                                static_cast<cudaStream_t>(cuda_stream)),
+                      "64x128 mask decode launch");
+}
+
 chorus_status chorus_visit_refresh(uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
                                    int group, void* cuda_stream) {
     g_err[0] = 0;
@@ -184,12 +215,33 @@ chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, con
                                                     lse, 0, 1.0f, cuda_stream);
 }
 
+static chorus_status attn_impl(const void* Q, const void* K, const void* V, const int32_t* row_ptr,
+                               const int32_t* col_idx, float scale, chorus_dtype dtype, void* O,
+                               const chorus_attn_shape* shape, const chorus_fp8_scales* fp8, float* lse,
+                               int n_first, float beta, bool half_flags, void* cuda_stream);
+
 chorus_status chorus_block_sparse_attn_fwd_first_frame(const void* Q, const void* K, const void* V,
                                                        const int32_t* row_ptr, const int32_t* col_idx,
                                                        float scale, chorus_dtype dtype, void* O,
                                                        const chorus_attn_shape* shape,
                                                        const chorus_fp8_scales* fp8, float* lse,
                                                        int n_first, float beta, void* cuda_stream) {
+    return attn_impl(Q, K, V, row_ptr, col_idx, scale, dtype, O, shape, fp8, lse, n_first, beta, false, cuda_stream);
+}
+
+chorus_status chorus_block_sparse_attn_fwd_64x128(const void* Q, const void* K, const void* V,
+                                                  const int32_t* row_ptr, const int32_t* col_idx,
+                                                  float scale, chorus_dtype dtype, void* O,
+                                                  const chorus_attn_shape* shape,
+                                                  const chorus_fp8_scales* fp8, float* lse,
+                                                  void* cuda_stream) {
+    return attn_impl(Q, K, V, row_ptr, col_idx, scale, dtype, O, shape, fp8, lse, 0, 1.0f, true, cuda_stream);
+}
+
+static chorus_status attn_impl(const void* Q, const void* K, const void* V, const int32_t* row_ptr,
+                               const int32_t* col_idx, float scale, chorus_dtype dtype, void* O,
+                               const chorus_attn_shape* shape, const chorus_fp8_scales* fp8, float* lse,
+                               int n_first, float beta, bool half_flags, void* cuda_stream) {
     g_err[0] = 0;
     if (n_first < 0) return set_error(CHORUS_ERR_INVALID_ARG, "n_first = %d is negative", n_first);
     if (!(beta > 0.f) || !(beta <= 3.0e38f))
@@ -235,6 +287,7 @@ chorus_status chorus_block_sparse_attn_fwd_first_frame(const void* Q, const void
     p.lse = lse;
     p.n_first = n_first < s.N ? n_first : s.N;
     p.beta = beta;
+    p.half_flags = half_flags;
     cudaError_t e = launch_attn_fwd(tmQ, tmK, tmV, tmO, p, dtype, static_cast<cudaStream_t>(cuda_stream));
     if (e == cudaErrorNotSupported)
         return set_error(CHORUS_ERR_UNSUPPORTED, "dtype %d not implemented by this build", (int)dtype);

@@ -18,6 +18,9 @@ size_t decode_workspace_bytes(int64_t rows, int words);
 cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, int words,
                                int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
                                cudaStream_t stream);
+size_t decode_64x128_workspace_bytes(int64_t heads, int N);
+cudaError_t launch_mask_decode_64x128(const uint32_t* bm64, int64_t heads, int N, int32_t* row_ptr,
+                                      int32_t* col_idx, int64_t col_cap, void* workspace, cudaStream_t stream);
 cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_layer, int words,
                                  int nk, int group, cudaStream_t stream);
 
@@ -47,6 +50,7 @@ struct AttnParams {
     float* lse;  // optional [B][H][N] row log-sum-exp (natural log), or null
     int n_first;  // first-frame key enhancement (eq. 1): scores of keys < n_first are multiplied by beta
     float beta;   // > 0; n_first = 0 or beta = 1 selects the plain kernel
+    bool half_flags;  // col_idx entries carry bits 30 / 31 (chorus_mask_to_index_64x128)
 };
 cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,

@@ -229,6 +229,57 @@ visit_refresh_kernel(uint32_t* __restrict__ bitmask, int n_groups, int64_t words
 }
 
 // one word per thread below this many words (a few layers), four above
+// ---- masks in the paper's 64 x 128 geometry (include/chorus.h) ---------------------
+// Step 1: the 64-key-tile mask of every 128-row block = union of its two 64-row mask rows, each key
+// block (128 keys) spread over its two tiles.  One thread per output word.
+__device__ __forceinline__ uint32_t spread16(uint32_t x) {      // bit b of the low 16 -> bits 2b, 2b+1
+    x = (x | (x << 8)) & 0x00ff00ffu;
+    x = (x | (x << 4)) & 0x0f0f0f0fu;
+    x = (x | (x << 2)) & 0x33333333u;
+    x = (x | (x << 1)) & 0x55555555u;
+    return x | (x << 1);
+}
+__global__ void __launch_bounds__(256)
+union_tiles_kernel(const uint32_t* __restrict__ bm64, int64_t heads /* L*H */, int nq64, int nq128,
+                   int nk128, int words128, int words64, uint32_t* __restrict__ out) {
+    const int64_t total = heads * nq128 * words64;
+    for (int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < total;
+         i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+        const int wo = static_cast<int>(i % words64);
+        const int64_t R = i / words64;
+        const int qb = static_cast<int>(R % nq128);
+        const int64_t hd = R / nq128;
+        const int wi = wo >> 1;
+        const uint32_t* up = bm64 + (hd * nq64 + 2 * qb) * words128;
+        uint32_t u = up[wi];
+        if (2 * qb + 1 < nq64) u |= up[words128 + wi];
+        const int rem = nk128 - wi * 32;                        // valid key blocks of this word
+        if (rem < 32) u &= (1u << rem) - 1u;
+        out[i] = spread16((u >> (16 * (wo & 1))) & 0xffffu);
+    }
+}
+
+// Step 3 (step 2 is the plain decode of that mask): one warp per 128-row block marks, in every entry,
+// which of its two halves does NOT keep the tile's key block.
+__global__ void __launch_bounds__(256)
+half_flags_kernel(const uint32_t* __restrict__ bm64, int64_t rows128, int nq64, int nq128, int words128,
+                  const int32_t* __restrict__ row_ptr, int32_t* __restrict__ col_idx, int64_t col_cap) {
+    const int64_t R = (static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
+    if (R >= rows128) return;
+    const int lane = threadIdx.x & 31;
+    const int qb = static_cast<int>(R % nq128);
+    const int64_t hd = R / nq128;
+    const uint32_t* up = bm64 + (hd * nq64 + 2 * qb) * words128;
+    const bool has_lo = 2 * qb + 1 < nq64;
+    const int64_t e1 = min(static_cast<int64_t>(row_ptr[R + 1]), col_cap);
+    for (int64_t e = row_ptr[R] + lane; e < e1; e += 32) {
+        const int t = col_idx[e], kb = t >> 1;
+        const uint32_t ku = (up[kb >> 5] >> (kb & 31)) & 1u;
+        const uint32_t kl = has_lo ? (up[words128 + (kb >> 5)] >> (kb & 31)) & 1u : 0u;
+        col_idx[e] = static_cast<int32_t>(static_cast<uint32_t>(t) | ((ku ^ 1u) << 30) | ((kl ^ 1u) << 31));
+    }
+}
+
 constexpr int64_t SMALL_WORDS = 1 << 20;
 inline int wpt_for(int64_t n_words) { return n_words < SMALL_WORDS ? 1 : 4; }
 inline int64_t n_tiles_for(int64_t rows, int words) {
@@ -268,6 +319,34 @@ cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_lay
     const int blocks = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 16));
     visit_refresh_kernel<<<blocks, 256, 0, stream>>>(bitmask, n_groups, words_per_layer, words, nk,
                                                      group);
+    count_launch(1);
+    return cudaGetLastError();
+}
+
+size_t decode_64x128_workspace_bytes(int64_t heads, int N) {
+    const int nq128 = (N + 127) / 128, words64 = ((N + 63) / 64 + 31) / 32;
+    const size_t un = (static_cast<size_t>(heads) * nq128 * words64 * 4 + 15) & ~size_t(15);
+    return un + decode_workspace_bytes(heads * nq128, words64);
+}
+
+cudaError_t launch_mask_decode_64x128(const uint32_t* bm64, int64_t heads, int N, int32_t* row_ptr,
+                                      int32_t* col_idx, int64_t col_cap, void* workspace, cudaStream_t stream) {
+    const int nq64 = (N + 63) / 64, nq128 = (N + 127) / 128, nk128 = nq128, nk64 = nq64;
+    const int words128 = (nk128 + 31) / 32, words64 = (nk64 + 31) / 32;
+    const int64_t rows128 = heads * nq128;
+    uint32_t* un = static_cast<uint32_t*>(workspace);
+    const size_t un_bytes = (static_cast<size_t>(rows128) * words64 * 4 + 15) & ~size_t(15);
+    const int64_t total = rows128 * words64;
+    const int blocks = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 16));
+    union_tiles_kernel<<<blocks, 256, 0, stream>>>(bm64, heads, nq64, nq128, nk128, words128, words64, un);
+    count_launch(1);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    e = launch_mask_decode(un, rows128, nk64, words64, row_ptr, col_idx, col_cap,
+                           static_cast<char*>(workspace) + un_bytes, stream);
+    if (e != cudaSuccess || col_idx == nullptr) return e;
+    half_flags_kernel<<<static_cast<unsigned>((rows128 * 32 + 255) / 256), 256, 0, stream>>>(
+        bm64, rows128, nq64, nq128, words128, row_ptr, col_idx, col_cap);
     count_launch(1);
     return cudaGetLastError();
 }
