@@ -187,17 +187,20 @@ def visit_refresh(mask, nk, group=8):
     return m
 
 
-def block_mass(Q, K, scale, qblocks=None, n_threads=0):
+def block_mass(Q, K, scale, qblocks=None, n_threads=0, block=(128, 64)):
     """True (dense) attention mass per block pair: Q, K bf16-bit arrays
     [B][N][H][d] -> float64 [B][H][nq][nk]; every valid query row contributes exactly 1.
-    qblocks: only these query blocks are computed (the rest of the output is 0)."""
+    qblocks: only these query blocks are computed (the rest of the output is 0).
+    block: (query rows, keys) per block, (128, 64) or the paper's (64, 128)."""
     assert Q.dtype == K.dtype == np.uint16
     B, N, H, d = Q.shape
-    nq, nk = (N + BQ - 1) // BQ, (N + BK - 1) // BK
+    assert tuple(block) in ((128, 64), (64, 128))
+    nq, nk = (N + block[0] - 1) // block[0], (N + block[1] - 1) // block[1]
     out = np.zeros((B, H, nq, nk), dtype=np.float64)
     sel = _c(np.asarray([] if qblocks is None else qblocks), np.int32)
     lib().oracle_block_mass(_p(Q), _p(K), B, H, N, d, *_strides(Q), *_strides(K),
-                            C.c_double(scale), _p(out), C.c_int(sel.size), _p(sel), C.c_int(n_threads))
+                            C.c_double(scale), _p(out), C.c_int(sel.size), _p(sel), C.c_int(n_threads),
+                            C.c_int(block[0]), C.c_int(block[1]))
     return out
 
 

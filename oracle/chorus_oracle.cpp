@@ -427,9 +427,11 @@ void oracle_visit_refresh(uint32_t* mask, int L, int H, int nq, int nk, int grou
 void oracle_block_mass(const uint16_t* Q, const uint16_t* K, int B, int H, int N, int d,
                        int64_t q_sb, int64_t q_sn, int64_t q_sh, int64_t k_sb, int64_t k_sn,
                        int64_t k_sh, double scale, double* mass, int n_sel, const int32_t* sel_qb,
-                       int n_threads) {
+                       int n_threads, int bq, int bk) {
     // n_sel > 0: only the query blocks listed in sel_qb are computed (the others stay as they are)
-    const int nq = (N + 127) / 128, nk = (N + 63) / 64;
+    // block geometry bq x bk: 128 x 64 (default, bq <= 0) or the paper's 64 x 128
+    const int BQ = bq > 0 ? bq : 128, BK = bk > 0 ? bk : 64;
+    const int nq = (N + BQ - 1) / BQ, nk = (N + BK - 1) / BK;
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
 #endif
@@ -449,7 +451,7 @@ void oracle_block_mass(const uint16_t* Q, const uint16_t* K, int B, int H, int N
         std::vector<double> kd(static_cast<size_t>(N) * d), s(N), q(d);
         for (int j = 0; j < N; ++j)
             for (int c = 0; c < d; ++c) kd[static_cast<size_t>(j) * d + c] = bf16_to_double(K[b * k_sb + j * k_sn + h * k_sh + c]);
-        for (int i = qb * 128; i < N && i < qb * 128 + 128; ++i) {
+        for (int i = qb * BQ; i < N && i < qb * BQ + BQ; ++i) {
             for (int c = 0; c < d; ++c) q[c] = bf16_to_double(Q[b * q_sb + i * q_sn + h * q_sh + c]);
             double m = -std::numeric_limits<double>::infinity();
             for (int j = 0; j < N; ++j) {
@@ -463,7 +465,7 @@ void oracle_block_mass(const uint16_t* Q, const uint16_t* K, int B, int H, int N
                 s[j] = std::exp(s[j] - m);
                 l += s[j];
             }
-            for (int j = 0; j < N; ++j) out[j / 64] += s[j] / l;
+            for (int j = 0; j < N; ++j) out[j / BK] += s[j] / l;
         }
     }
 }

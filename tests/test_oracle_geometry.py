@@ -98,3 +98,29 @@ def test_decode_64x128_matches_brute_force_and_round_trips(N):
                 assert np.all(np.diff(tiles.astype(np.int64)) > 0)           # ascending, no duplicates
             ref = np.repeat(np.repeat(keep[l, h], 64, axis=0), 128, axis=1)[:N, :N]
             assert np.array_equal(tok, ref)
+
+
+def test_block_mass_64x128_equals_numpy_softmax_summed_per_block():
+    """oracle.block_mass(block=(64, 128)) against numpy: the dense softmax matrix summed over 64-row x 128-key
+    blocks; it is also the 128 x 64 result regrouped where both geometries tile evenly."""
+    N, H = 449, 2
+    Q, K, _ = random_qkv_bits(N, H, seed=12)
+    m = oracle.block_mass(Q, K, SCALE, block=(64, 128))
+    nq64, nk128 = (N + 63) // 64, (N + 127) // 128
+    assert m.shape == (1, H, nq64, nk128)
+    for h in range(H):
+        q, k = bits_to_f64(Q[0, :, h]), bits_to_f64(K[0, :, h])
+        s = SCALE * (q @ k.T)
+        p = np.exp(s - s.max(axis=1, keepdims=True))
+        p /= p.sum(axis=1, keepdims=True)
+        ref = np.zeros((nq64, nk128))
+        for i in range(N):
+            for kb in range(nk128):
+                ref[i // 64, kb] += p[i, 128 * kb: 128 * kb + 128].sum()
+        np.testing.assert_allclose(m[0, h], ref, rtol=0, atol=1e-12)
+        np.testing.assert_allclose(m[0, h].sum(axis=1), np.minimum(64, N - 64 * np.arange(nq64)), rtol=1e-12)
+    # token-level consistency of the two geometries: both sum to the same 128 x 128 super-blocks
+    m2 = oracle.block_mass(Q, K, SCALE)                              # [1][H][4][8]
+    a = m[0, :, : 2 * (nq64 // 2)].reshape(H, nq64 // 2, 2, nk128).sum(axis=2)
+    b = np.pad(m2[0], ((0, 0), (0, 0), (0, 2 * nk128 - m2.shape[3]))).reshape(H, m2.shape[2], nk128, 2).sum(axis=3)
+    np.testing.assert_allclose(a, b[:, : nq64 // 2], rtol=0, atol=1e-12)
