@@ -279,6 +279,14 @@ chorus_status chorus_retrieve_top1(const float* bank, int n, int dim, const floa
 chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
                                 const chorus_attn_shape* shape, const float* lse, float* mass,
                                 void* cuda_stream);
+/* chorus_block_mass with its output in the paper's 64 x 128 geometry (R26):
+ * mass is float [B][H][ceil(N/64)][ceil(N/128)], mass[b][h][qb][kb] = sum of the token-level
+ * probabilities of query rows 64 qb .. 64 qb + 63 over keys 128 kb .. 128 kb + 127.  Everything else
+ * as chorus_block_mass; chorus_mask_from_mass (rows = B*H*ceil(N/64), nk_blk = ceil(N/128)) then
+ * gives the bitmask chorus_mask_to_index_64x128 reads. */
+chorus_status chorus_block_mass_64x128(const void* Q, const void* K, float scale,
+                                       const chorus_attn_shape* shape, const float* lse, float* mass,
+                                       void* cuda_stream);
 chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk, float top_p,
                                     float min_top_k, uint32_t* bitmask, int32_t* kept,
                                     void* cuda_stream);

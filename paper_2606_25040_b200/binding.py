@@ -20,7 +20,7 @@ BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
 
 EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
            "chorus_block_sparse_attn_fwd_lse", "chorus_block_sparse_attn_fwd_first_frame",
-           "chorus_mask_to_index_64x128", "chorus_block_sparse_attn_fwd_64x128",
+           "chorus_mask_to_index_64x128", "chorus_block_sparse_attn_fwd_64x128", "chorus_block_mass_64x128",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
            "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count"]
@@ -70,6 +70,7 @@ def lib() -> C.CDLL:
                                            C.POINTER(C.c_size_t), C.c_void_p]
         L.chorus_block_mass.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.POINTER(AttnShape),
                                         C.c_void_p, C.c_void_p, C.c_void_p]
+        L.chorus_block_mass_64x128.argtypes = L.chorus_block_mass.argtypes
         L.chorus_block_sparse_attn_fwd_lse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                                        C.c_void_p, C.c_float, C.c_int, C.c_void_p,
                                                        C.POINTER(AttnShape), C.POINTER(Fp8Scales),
@@ -286,16 +287,19 @@ def chorus_retrieve_top1(bank, query, tau: float, out=None, workspace=None, stre
     return out
 
 
-def chorus_block_mass(Q, K, scale: float, mass=None, stream=None, lse=None):
+def chorus_block_mass(Q, K, scale: float, mass=None, stream=None, lse=None, geometry_64x128=False):
     """bf16 Q, K [B][N][H][d] (cuda) -> float32 mass [B][H][ceil(N/128)][ceil(N/64)] of the dense
-    attention (PAPER.md:L73, L81)."""
+    attention (PAPER.md:L73, L81); geometry_64x128: [B][H][ceil(N/64)][ceil(N/128)] (chorus_block_mass_64x128)."""
     B, N, H, d = Q.shape
     nq, nk = (N + BLOCK_Q - 1) // BLOCK_Q, (N + BLOCK_K - 1) // BLOCK_K
+    if geometry_64x128:
+        nq, nk = nk, nq
     if mass is None:
         mass = torch.empty((B, H, nq, nk), dtype=torch.float32, device=Q.device)
+    assert mass.shape == (B, H, nq, nk) and mass.is_contiguous() and mass.dtype == torch.float32
     shape = attn_shape(Q, K, K)
-    _check(lib().chorus_block_mass(_ptr(Q), _ptr(K), C.c_float(scale), C.byref(shape), _ptr(lse),
-                                   _ptr(mass), _stream(stream)))
+    fn = lib().chorus_block_mass_64x128 if geometry_64x128 else lib().chorus_block_mass
+    _check(fn(_ptr(Q), _ptr(K), C.c_float(scale), C.byref(shape), _ptr(lse), _ptr(mass), _stream(stream)))
     return mass
 
 

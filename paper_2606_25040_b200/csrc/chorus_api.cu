@@ -294,9 +294,23 @@ static chorus_status attn_impl(const void* Q, const void* K, const void* V, cons
     return check_cuda(e, "attention launch");
 }
 
+static chorus_status block_mass_impl(const void* Q, const void* K, float scale, const chorus_attn_shape* shape,
+                                     const float* lse, float* mass, bool geo64, void* cuda_stream);
+
 chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
                                 const chorus_attn_shape* shape, const float* lse, float* mass,
                                 void* cuda_stream) {
+    return block_mass_impl(Q, K, scale, shape, lse, mass, false, cuda_stream);
+}
+
+chorus_status chorus_block_mass_64x128(const void* Q, const void* K, float scale,
+                                       const chorus_attn_shape* shape, const float* lse, float* mass,
+                                       void* cuda_stream) {
+    return block_mass_impl(Q, K, scale, shape, lse, mass, true, cuda_stream);
+}
+
+static chorus_status block_mass_impl(const void* Q, const void* K, float scale, const chorus_attn_shape* shape,
+                                     const float* lse, float* mass, bool geo64, void* cuda_stream) {
     g_err[0] = 0;
     if (!Q || !K || !mass) return set_error(CHORUS_ERR_INVALID_ARG, "Q, K, mass must be non-null");
     if (!aligned16(Q) || !aligned16(K)) return set_error(CHORUS_ERR_INVALID_ARG, "Q, K must be 16-byte aligned");
@@ -311,7 +325,7 @@ chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
                         64, 128, "Q")) != CHORUS_OK) return st;
     if ((st = make_tmap(&tmK, K, 2, s.B, s.H, s.N, s.d, s.k_stride_b, s.k_stride_n, s.k_stride_h,
                         64, 128, "K")) != CHORUS_OK) return st;
-    return check_cuda(launch_block_mass(tmQ, tmK, lse, mass, s.B, s.H, s.N, scale * 1.4426950408889634f,
+    return check_cuda(launch_block_mass(tmQ, tmK, lse, mass, s.B, s.H, s.N, scale * 1.4426950408889634f, geo64,
                                         static_cast<cudaStream_t>(cuda_stream)), "block mass launch");
 }
 

@@ -58,7 +58,7 @@ cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, cons
 
 // ---- mask_build.cu -----------------------------------------------------------------------------
 cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, const float* lse, float* mass,
-                              int B, int H, int N, float scale_log2, cudaStream_t stream);
+                              int B, int H, int N, float scale_log2, bool geo64, cudaStream_t stream);
 cudaError_t launch_mask_from_mass(const float* mass, int64_t rows, int nk, double top_p, double min_top_k,
                                   uint32_t* bitmask, int32_t* kept, cudaStream_t stream);
 cudaError_t launch_mask_coverage(const float* mass, const uint32_t* bitmask, int heads, int nq, int nk,

@@ -46,6 +46,7 @@ struct MassParams {
     const float* lse;   // optional [B][H][N] natural-log row log-sum-exp of the SAME dense attention
     int B, H, N, nq, nk;
     float scale_log2;
+    int geo64;          // 1: output in the paper's 64 x 128 geometry, [B][H][ceil(N/64)][ceil(N/128)]
 };
 
 template <bool kLse>   // the rows' log-sum-exp is given: one pass over the keys instead of two
@@ -214,9 +215,19 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     if (wq == 0 && lane == 0) {
                         const float a = ((part[0] + part[2]) + part[4]) + part[6];
                         const float bsum = ((part[1] + part[3]) + part[5]) + part[7];
+                        if (p.geo64) {
+                            // 64 x 128 geometry: step j is key block j; warps 0-1 / 2-3 hold rows 0-63 / 64-127
+                            const int nq64 = (p.N + 63) >> 6, nk128 = p.nq;
+                            const int qb = idx % p.nq;
+                            const int64_t bh = idx / p.nq;
+                            float* out = p.mass + (bh * nq64 + 2 * qb) * nk128 + j;
+                            out[0] = (part[0] + part[2]) + (part[1] + part[3]);
+                            if (2 * qb + 1 < nq64) out[nk128] = (part[4] + part[6]) + (part[5] + part[7]);
+                        } else {
                         float* out = p.mass + static_cast<int64_t>(idx) * p.nk + 2 * j;
                         out[0] = a;
                         if (2 * j + 1 < p.nk) out[1] = bsum;
+                        }
                     }
                     ++own;
                 }
@@ -356,7 +367,7 @@ mask_coverage_kernel(const float* __restrict__ mass, const uint32_t* __restrict_
 }  // namespace
 
 cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, const float* lse, float* mass,
-                              int B, int H, int N, float scale_log2, cudaStream_t stream) {
+                              int B, int H, int N, float scale_log2, bool geo64, cudaStream_t stream) {
     cudaError_t e = lse ? cudaFuncSetAttribute(block_mass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, M_SMEM)
                         : cudaFuncSetAttribute(block_mass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, M_SMEM);
     if (e != cudaSuccess) return e;
@@ -370,6 +381,7 @@ cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, co
     p.nq = (N + 127) / 128;
     p.nk = (N + 63) / 64;
     p.scale_log2 = scale_log2;
+    p.geo64 = geo64 ? 1 : 0;
     const int n_items = B * H * p.nq;
     const int grid = n_items < sms ? n_items : sms;
     if (lse) block_mass_kernel<true><<<grid, MB_THREADS, M_SMEM, stream>>>(tmQ, tmK, p);

@@ -159,3 +159,46 @@ def test_cfg2_full_size_sampled_blocks_64x128():
     (mx, mean, relfro, _), _, _ = compare_items(O.float().cpu().numpy().astype(np.float64), Q, K, V, bm[0], N, H,
                                                 items=items)
     assert mx <= BF16_MAX and mean <= BF16_MEAN and relfro <= BF16_RELFRO, (mx, mean, relfro)
+
+
+@pytest.mark.parametrize("N,H,scale", [(512, 2, 0.0884), (200, 1, 0.3), (1000, 3, 0.0884), (64, 1, 1.0), (449, 2, 0.5)])
+def test_block_mass_64x128_matches_oracle_and_closes_the_loop(N, H, scale):
+    """chorus_block_mass_64x128 (two passes and one pass with the LSE) against the oracle; then the paper-geometry
+    loop on the GPU alone: mass -> top-p mask (bit-exact against the oracle on the same masses) -> 64 x 128 index
+    -> attention, compared with the oracle on that mask."""
+    g = np.random.default_rng(N)
+    Q, K, V = (W.bf16_bits_from_f32(g.standard_normal((1, N, H, 128)).astype(np.float32)) for _ in range(3))
+    scale = float(np.float32(scale))
+    ref = oracle.block_mass(Q, K, scale, block=(64, 128))
+    q, k, v = dbf16(Q), dbf16(K), dbf16(V)
+    got = B.chorus_block_mass(q, k, scale, geometry_64x128=True)
+    # one pass, with the row log-sum-exp of the dense attention call
+    nk64 = (N + 63) // 64
+    full = torch.full((1, H, (N + 127) // 128, (nk64 + 31) // 32), -1, dtype=torch.int32, device=dev())
+    rp, ci = B.chorus_mask_to_index(full, nk64)
+    lse = torch.empty((1, H, N), dtype=torch.float32, device=dev())
+    B.chorus_block_sparse_attn_fwd(q, k, v, rp, ci, scale, lse=lse)
+    got1 = B.chorus_block_mass(q, k, scale, lse=lse, geometry_64x128=True)
+    torch.cuda.synchronize()
+    for m in (got, got1):
+        m = m.cpu().numpy().astype(np.float64)
+        assert m.shape == ref.shape
+        tol = 2e-3 * np.maximum(ref, 1e-3) + 1e-5
+        assert np.all(np.abs(m - ref) <= tol), float(np.abs(m - ref).max())
+    bm, kept = B.chorus_mask_from_mass(got[0], 0.9, 0.1)
+    torch.cuda.synchronize()
+    bm_o, kept_o = oracle.mask_from_mass(got[0].cpu().numpy(), ref.shape[3], float(np.float32(0.9)), float(np.float32(0.1)))
+    assert np.array_equal(bm.cpu().numpy().view(np.uint32), bm_o) and np.array_equal(kept.cpu().numpy(), kept_o)
+    rp2, ci2 = B.chorus_mask_to_index_64x128(bm[None], N)
+    O = B.chorus_block_sparse_attn_fwd(q, k, v, rp2, ci2, scale, geometry_64x128=True)
+    torch.cuda.synchronize()
+    nq64 = (N + 63) // 64
+    items = [(0, h, qb) for h in range(H) for qb in range(nq64)]
+    refO = oracle.block_sparse_attn(Q, K, V, bm_o, scale, items=np.asarray(items, np.int32), block=(64, 128))
+    Of = O.float().cpu().numpy().astype(np.float64)
+    gotO = np.zeros_like(refO)
+    for t, (_, h, qb) in enumerate(items):
+        lo, hi = 64 * qb, min(N, 64 * qb + 64)
+        gotO[t, : hi - lo] = Of[0, lo:hi, h]
+    mx, mean, _, _ = err_stats(gotO, refO)
+    assert mx <= BF16_MAX and mean <= BF16_MEAN, (mx, mean)
