@@ -14,7 +14,11 @@
 //   oracle_mask_to_index        pinned (brute force, popcount total, round trip, word-boundary cases)
 //   oracle_block_sparse_attn    pinned (numpy dense fp64 softmax for full/diagonal/single-block masks,
 //                               long-double brute force with materialised -inf scores, closed forms,
-//                               hand-derived golden fixture, permutation invariance, padded tail)
+//                               hand-derived golden fixture, permutation invariance, padded tail);
+//                               first-frame key scaling (eq. 1): numpy dense attention on hand-scaled
+//                               keys, closed form; 64 x 128 geometry: numpy token-level masked softmax
+//   oracle_mask_to_index_64x128 pinned (brute-force restatement, round trip to the token-level keep
+//                               matrix of the mask, ascending / no duplicates)
 //   oracle_quantize_fp8         pinned (torch.float8_e4m3fn cast as an independent library routine,
 //                               error bound, exact round trip of {0, +-amax}); the FORMAT itself
 //                               (granularity, amax/448) is reading R10/R11 — the paper only says
@@ -23,7 +27,8 @@
 //   oracle_retrieve_top1        pinned (planted neighbour, numpy argmax)
 //   oracle_visit_refresh        pinned (brute force per bit, every pair visited once per group)
 //   oracle_block_mass           pinned (numpy dense softmax summed per block, rows sum to 1, uniform
-//                               attention closed form)
+//                               attention closed form; 64 x 128 geometry: numpy, and agreement of
+//                               the two geometries on 128 x 128 super-blocks)
 //   oracle_mask_from_mass       pinned (exact-rational brute force on tiny rows, minimality of the
 //                               kept prefix, floor count, ties by index, hand-worked golden row)
 //   oracle_mask_coverage        pinned (numpy; full mask = 1, top-p mask >= p)

@@ -1,0 +1,90 @@
+"""Timing of the attention variants of row f-4 on the 480p layer:
+
+    python -m paper_2606_25040_b200.bench_variants [--iters K]
+
+Prints one JSON line: the plain BF16 / FP8 calls, the same with first-frame key enhancement (PAPER.md:L109-114
+eq. (1), n_first = 1560, beta = 1.2), and the paper's 64 x 128 mask geometry with a 25 % mask
+whose row pairs agree / are independent, plus the 64 x 128 decode.  CUDA events, median of K launches; inputs
+(1.34 GB) exceed L2.  bench.py stays the headline benchmark.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import statistics
+
+import numpy as np
+import torch
+
+from . import binding as B
+from . import workloads as W
+
+
+def _time(fn, iters):
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(iters):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    return statistics.median(ts)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--iters", type=int, default=10)
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("needs a CUDA device (no CPU fallback)")
+    dev = torch.device("cuda:0")
+    cfg = W.CFG2
+    N, H = cfg.N, cfg.H
+    g = torch.Generator(device=dev)
+    g.manual_seed(0)
+    Q, K, V = (torch.randn((1, N, H, cfg.d), device=dev, generator=g).to(torch.bfloat16) for _ in range(3))
+    O = torch.empty_like(Q)
+    qz = B.chorus_quantize_fp8(Q, K, V)
+    bm = torch.from_numpy(W.layer_mask(cfg)[None].view(np.int32)).to(dev)
+    rp, ci = B.chorus_mask_to_index(bm, cfg.nk)
+    out = {"workload": cfg.name, "H": H, "N": N, "density": cfg.density}
+
+    def bf16(**kw):
+        return _time(lambda: B.chorus_block_sparse_attn_fwd(Q, K, V, rp, ci, cfg.scale, O=O, **kw), args.iters)
+
+    def fp8(**kw):
+        return _time(lambda: B.chorus_block_sparse_attn_fwd(qz[0], qz[1], qz[2], rp, ci, cfg.scale, O=O,
+                                                            dtype=B.CHORUS_FP8_E4M3, fp8_scales=qz[3:], **kw),
+                     args.iters)
+
+    ff = dict(n_first=cfg.hp * cfg.wp, beta=1.2)
+    out["plain_bf16_ms"], out["plain_fp8_ms"] = bf16(), fp8()
+    out["first_frame_bf16_ms"], out["first_frame_fp8_ms"] = bf16(**ff), fp8(**ff)
+    out["first_frame"] = ff
+
+    # the paper's geometry: 64-row x 128-key mask blocks at 25 %
+    rng = np.random.default_rng(0)
+    nq64, nk128 = (N + 63) // 64, (N + 127) // 128
+    k_half = rng.random((H, nq64 // 2, nk128)) < 0.25
+    cases = (("halves_agree", np.repeat(k_half, 2, axis=1)), ("halves_independent", rng.random((H, nq64, nk128)) < 0.25))
+    for name, keep in cases:
+        bm64 = torch.from_numpy(W.pack_bits(keep)[None].view(np.int32)).to(dev)
+        rp64, ci64 = B.chorus_mask_to_index_64x128(bm64, N)
+        t_dec = _time(lambda: B.chorus_mask_to_index_64x128(bm64, N, row_ptr=rp64, col_idx=ci64), args.iters)
+        t_att = _time(lambda: B.chorus_block_sparse_attn_fwd(Q, K, V, rp64, ci64, cfg.scale, O=O,
+                                                             geometry_64x128=True), args.iters)
+        tiles = int(rp64[-1])
+        out["geometry_64x128_" + name] = {
+            "mask_density": float(keep.mean()), "tiles_computed_frac": tiles / (H * cfg.nq * cfg.nk),
+            "decode_us": t_dec * 1e3, "attn_bf16_ms": t_att,
+            "TFLOPs_on_computed_tiles": 4.0 * 128 * 64 * 128 * tiles / (t_att * 1e-3) / 1e12,
+            "TFLOPs_on_mask_blocks": 4.0 * 64 * 128 * 128 * float(keep.sum()) / (t_att * 1e-3) / 1e12}
+    print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()
