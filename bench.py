@@ -314,7 +314,7 @@ def run_chorus(args):
     # The host tensors are stored head-major ([B][H][N][d]; the ABI takes it through its strides), so
     # that a group of heads is one contiguous copy: heads go through in E2E_CHUNKS groups on three
     # streams (H2D of group c+1 | the kernels of group c | D2H of group c-1).  Same bytes, same calls.
-    E2E_CHUNKS = 8 if cfg.H % 8 == 0 else 1
+    E2E_CHUNKS = next(c for c in (20, 10, 8, 5, 4, 2, 1) if cfg.H % c == 0)   # small groups: short fill and drain
     hc = cfg.H // E2E_CHUNKS
     hm = lambda t: t.permute(0, 2, 1, 3).contiguous()                 # [B][N][H][d] -> [B][H][N][d]
     hQh, hKh, hVh = (hm(x).pin_memory() for x in (hQ, hK, hV))
@@ -326,12 +326,19 @@ def run_chorus(args):
     s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
     ev_in = [torch.cuda.Event() for _ in range(E2E_CHUNKS)]
     ev_done = [torch.cuda.Event() for _ in range(E2E_CHUNKS)]
-    ev_top = torch.cuda.Event()
+    ev_top, ev_mask = torch.cuda.Event(), torch.cuda.Event()
+    ev_h2d = [torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)]
 
     def e2e_step():
         ev_top.record(stream)
         s_in.wait_event(ev_top)                 # do not run ahead of the step's start
-        dM.copy_(hM, non_blocking=True)
+        ev_h2d[0].record(s_in)
+        # every host-to-device copy goes on s_in: a copy issued on the compute stream sits in the same
+        # copy-engine queue as the Q/K/V groups and cost 2 ms per step
+        with torch.cuda.stream(s_in):
+            dM.copy_(hM, non_blocking=True)
+            ev_mask.record(s_in)
+        stream.wait_event(ev_mask)
         B.chorus_mask_to_index(dM, cfg.nk, row_ptr=row_ptr, col_idx=col_idx, workspace=ws)
         for c in range(E2E_CHUNKS):
             hs = slice(c * hc, (c + 1) * hc)
@@ -353,6 +360,7 @@ def run_chorus(args):
             with torch.cuda.stream(s_out):
                 s_out.wait_event(ev_done[c])
                 hOh[:, hs].copy_(dOh[:, hs], non_blocking=True)
+        ev_h2d[1].record(s_in)
         stream.wait_stream(s_out)               # the step ends when its result is in host memory
         stream.wait_stream(s_in)
 
@@ -361,11 +369,14 @@ def run_chorus(args):
     barrier()
     a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(stream)
+    t_host = time.perf_counter()
     for _ in range(e2e_steps):
         e2e_step()
+    t_host = (time.perf_counter() - t_host) / e2e_steps * 1e3      # host time to enqueue one step
     b_.record(stream)
     barrier()
     e2e_ms = a.elapsed_time(b_) / e2e_steps
+    e2e_h2d_ms = ev_h2d[0].elapsed_time(ev_h2d[1])     # the last step's host-to-device copies, first to last
     # the pipelined path must give what the single call gives
     e2e_ok = bool(torch.equal(hOh.permute(0, 2, 1, 3), dO.cpu())) if rank == 0 else True
 
@@ -451,7 +462,7 @@ def run_chorus(args):
                        "l2": "inputs larger than L2 (Q+K+V+O = %.2f GB per step)" % (4 * Qb.nbytes / 1e9),
                        "step": "mask_to_index -> attn_fwd(bf16)" + (" -> quantize_fp8 -> attn_fwd(fp8)" if has_fp8 else "")},
             "clocks": clocks,
-            "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms,
+            "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_span_ms": e2e_h2d_ms, "host_enqueue_ms": t_host,
                     "h2d_bytes_per_step": int(3 * Qb.nbytes + bm.nbytes), "d2h_bytes_per_step": int(Qb.nbytes),
                     "pipeline": "%d head groups, H2D | kernels | D2H on three streams, head-major host tensors" % E2E_CHUNKS,
                     "matches_single_call": e2e_ok},
