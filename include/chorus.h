@@ -20,6 +20,7 @@
  *                                 dense attention mass per block -> top-p mask with a top-k floor
  *                                 -> coverage                                                  (L73, L81, L93 (2))
  *   chorus_head_costs / chorus_schedule_heads   per-head cost and greedy head -> rank schedule (L95, appendix A)
+ *   chorus_gather_heads / chorus_scatter_heads  the local copies around the Ulysses all-to-all   (L95, appendix A)
  *
  * Conventions (all entry points)
  *   - Plain C: pointers and sizes only.  "device" = pointer into CUDA device memory of the current
@@ -313,6 +314,29 @@ chorus_status chorus_head_costs(const int32_t* row_ptr, int H, int nq_blk, int64
                                 void* cuda_stream);
 chorus_status chorus_schedule_heads(const int64_t* cost, int H, int n_ranks, int32_t* order,
                                     int64_t* load);
+
+/* ---------------------------------------------------------------------------------------------
+ * The two local copies around the Ulysses all-to-all (appendix A: the heads
+ * are "re-partitioned (reordered) across ranks before the all-to-all communication").  A rank of a
+ * sequence-parallel group holds n_tokens tokens of all H heads; the exchange hands rank p the heads
+ * order[p * slots .. (p + 1) * slots), slots = H / n_ranks, of every rank's tokens.
+ *   chorus_gather_heads    packed[p][i][s][:] = X[i][order[p * slots + s]][:]      (before the exchange)
+ *   chorus_scatter_heads   X[i][order[p * slots + s]][:] = packed[p][i][s][:]      (after it, for O)
+ * X        device, [n_tokens][H][d] with element strides stride_n, stride_h (last dim contiguous).
+ * packed   device, contiguous [n_ranks][n_tokens][slots][d]: chunk p is what goes to / came from rank p.
+ * order    HOST, H head indices, a permutation of 0..H-1 (chorus_schedule_heads' `order` when
+ *          H % n_ranks == 0); validated on the host.
+ * elem_bytes 1, 2 or 4; d * elem_bytes and the strides in bytes must be multiples of 16; X and packed
+ *          16-byte aligned.  The exchange itself is the caller's (NCCL all-to-all with equal splits;
+ *          paper_2606_25040_b200/ulysses.py); with one rank both calls are a head permutation.
+ * Bit-exact copies.  Errors: INVALID_ARG, UNSUPPORTED (H > 256), CUDA.
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_gather_heads(const void* X, int n_tokens, int H, int d, int elem_bytes, int64_t stride_n,
+                                  int64_t stride_h, const int32_t* order, int n_ranks, void* packed,
+                                  void* cuda_stream);
+chorus_status chorus_scatter_heads(const void* packed, int n_tokens, int H, int d, int elem_bytes,
+                                   int64_t stride_n, int64_t stride_h, const int32_t* order, int n_ranks,
+                                   void* X, void* cuda_stream);
 
 /* Thread-local description of the last error returned on this thread ("" if none). */
 const char* chorus_last_error(void);

@@ -247,3 +247,25 @@ def schedule_heads(cost, n_ranks):
         mine[best].append(h)
         load[best] += cost[h]
     return [sorted(m) for m in mine], load
+
+
+def gather_heads(X, order, n_ranks):
+    """PAPER.md:L95 / appendix A, the copy before the Ulysses all-to-all, written out: X [n][H][d] ->
+    packed [n_ranks][n][H/n_ranks][d] with packed[p][i][s] = X[i][order[p * slots + s]]."""
+    n, H, d = X.shape
+    slots = H // n_ranks
+    out = np.empty((n_ranks, n, slots, d), dtype=X.dtype)
+    for p in range(n_ranks):
+        for s in range(slots):
+            out[p, :, s, :] = X[:, int(order[p * slots + s]), :]
+    return out
+
+
+def scatter_heads(packed, order):
+    """The inverse copy: packed [n_ranks][n][slots][d] -> X [n][H][d]."""
+    n_ranks, n, slots, d = packed.shape
+    X = np.empty((n, n_ranks * slots, d), dtype=packed.dtype)
+    for p in range(n_ranks):
+        for s in range(slots):
+            X[:, int(order[p * slots + s]), :] = packed[p, :, s, :]
+    return X

@@ -22,7 +22,7 @@ EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_
            "chorus_block_sparse_attn_fwd_lse", "chorus_block_sparse_attn_fwd_first_frame",
            "chorus_mask_to_index_64x128", "chorus_block_sparse_attn_fwd_64x128", "chorus_block_mass_64x128",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
-           "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_last_error", "chorus_version",
+           "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_gather_heads", "chorus_scatter_heads", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count"]
 
 
@@ -84,6 +84,9 @@ def lib() -> C.CDLL:
                                             C.c_void_p, C.c_void_p, C.c_void_p]
         L.chorus_mask_coverage.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
                                            C.c_void_p, C.c_void_p]
+        L.chorus_gather_heads.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int64, C.c_int64,
+                                          C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.chorus_scatter_heads.argtypes = L.chorus_gather_heads.argtypes
         L.chorus_head_costs.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         L.chorus_schedule_heads.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         _lib = L
@@ -347,3 +350,36 @@ def chorus_schedule_heads(cost, n_ranks: int):
     load = torch.empty(n_ranks, dtype=torch.int64)
     _check(lib().chorus_schedule_heads(_ptr(cost), H, n_ranks, _ptr(order), _ptr(load)))
     return order, load
+
+
+def _host_order(order, H):
+    o = torch.as_tensor(order, dtype=torch.int32).reshape(-1).contiguous().cpu()
+    assert o.numel() == H, (o.numel(), H)
+    return o
+
+
+def chorus_gather_heads(X, order, n_ranks: int, packed=None, stream=None):
+    """X: cuda [n_tokens][H][d] (strided views are fine, last dim contiguous); order: H head indices (host).
+    Returns packed [n_ranks][n_tokens][H/n_ranks][d]: chunk p holds the heads order[p*slots:(p+1)*slots]."""
+    n, H, d = X.shape
+    assert X.is_cuda and X.stride(2) == 1
+    if packed is None:
+        packed = torch.empty(X.numel(), dtype=X.dtype, device=X.device)
+        if n_ranks > 0 and H % n_ranks == 0:          # otherwise the library reports the error
+            packed = packed.view(n_ranks, n, H // n_ranks, d)
+    assert packed.is_contiguous() and packed.dtype == X.dtype and packed.numel() == X.numel()
+    o = _host_order(order, H)
+    _check(lib().chorus_gather_heads(_ptr(X), n, H, d, X.element_size(), X.stride(0), X.stride(1), _ptr(o), n_ranks,
+                                     _ptr(packed), _stream(stream)))
+    return packed
+
+
+def chorus_scatter_heads(packed, order, X, stream=None):
+    """Inverse of chorus_gather_heads: packed [n_ranks][n_tokens][slots][d] -> X [n_tokens][H][d] (written)."""
+    n_ranks, n, slots, d = packed.shape
+    H = n_ranks * slots
+    assert packed.is_cuda and packed.is_contiguous() and X.shape == (n, H, d) and X.stride(2) == 1
+    o = _host_order(order, H)
+    _check(lib().chorus_scatter_heads(_ptr(packed), n, H, d, X.element_size(), X.stride(0), X.stride(1), _ptr(o),
+                                      n_ranks, _ptr(X), _stream(stream)))
+    return X

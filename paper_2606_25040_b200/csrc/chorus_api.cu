@@ -374,6 +374,45 @@ chorus_status chorus_schedule_heads(const int64_t* cost, int H, int n_ranks, int
     return CHORUS_OK;
 }
 
+static chorus_status move_heads(bool scatter, const void* src, void* dst, const int32_t* order, int n_tokens,
+                                int H, int n_ranks, int d, int elem_bytes, int64_t stride_n, int64_t stride_h,
+                                void* cuda_stream) {
+    g_err[0] = 0;
+    if (!src || !dst || !order) return set_error(CHORUS_ERR_INVALID_ARG, "X, packed, order must be non-null");
+    if (n_tokens < 0 || H <= 0 || n_ranks <= 0 || d <= 0)
+        return set_error(CHORUS_ERR_INVALID_ARG, "n_tokens >= 0 and H, n_ranks, d > 0 required");
+    if (H % n_ranks) return set_error(CHORUS_ERR_INVALID_ARG, "H = %d is not a multiple of n_ranks = %d", H, n_ranks);
+    if (H > CHORUS_MAX_EXCHANGE_HEADS) return set_error(CHORUS_ERR_UNSUPPORTED, "H = %d > %d", H, CHORUS_MAX_EXCHANGE_HEADS);
+    if (elem_bytes != 1 && elem_bytes != 2 && elem_bytes != 4)
+        return set_error(CHORUS_ERR_INVALID_ARG, "elem_bytes must be 1, 2 or 4");
+    const int64_t row_bytes = static_cast<int64_t>(d) * elem_bytes;
+    if (row_bytes % 16 || (stride_n * elem_bytes) % 16 || (stride_h * elem_bytes) % 16)
+        return set_error(CHORUS_ERR_INVALID_ARG, "rows and strides must be multiples of 16 bytes");
+    if (stride_h < d || stride_n < d) return set_error(CHORUS_ERR_INVALID_ARG, "strides smaller than a row");
+    if (!aligned16(src) || !aligned16(dst)) return set_error(CHORUS_ERR_INVALID_ARG, "X, packed must be 16-byte aligned");
+    bool seen[CHORUS_MAX_EXCHANGE_HEADS] = {false};
+    for (int k = 0; k < H; ++k) {
+        if (order[k] < 0 || order[k] >= H || seen[order[k]])
+            return set_error(CHORUS_ERR_INVALID_ARG, "order is not a permutation of 0..H-1 (entry %d = %d)", k, order[k]);
+        seen[order[k]] = true;
+    }
+    return check_cuda(launch_move_heads(scatter, src, dst, order, n_tokens, H, n_ranks, static_cast<int>(row_bytes),
+                                        stride_n * elem_bytes, stride_h * elem_bytes,
+                                        static_cast<cudaStream_t>(cuda_stream)), "head exchange copy launch");
+}
+
+chorus_status chorus_gather_heads(const void* X, int n_tokens, int H, int d, int elem_bytes, int64_t stride_n,
+                                  int64_t stride_h, const int32_t* order, int n_ranks, void* packed,
+                                  void* cuda_stream) {
+    return move_heads(false, X, packed, order, n_tokens, H, n_ranks, d, elem_bytes, stride_n, stride_h, cuda_stream);
+}
+
+chorus_status chorus_scatter_heads(const void* packed, int n_tokens, int H, int d, int elem_bytes,
+                                   int64_t stride_n, int64_t stride_h, const int32_t* order, int n_ranks,
+                                   void* X, void* cuda_stream) {
+    return move_heads(true, packed, X, order, n_tokens, H, n_ranks, d, elem_bytes, stride_n, stride_h, cuda_stream);
+}
+
 chorus_status chorus_quantize_fp8(const void* Q, const void* K, const void* V,
                                   const chorus_attn_shape* shape, void* q8, void* k8, void* v8,
                                   float* q_scale, float* k_scale, float* v_scale,

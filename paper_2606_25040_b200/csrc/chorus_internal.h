@@ -66,6 +66,11 @@ cudaError_t launch_mask_coverage(const float* mass, const uint32_t* bitmask, int
 
 // ---- head_schedule.cu --------------------------------------------------------------------------
 cudaError_t launch_head_costs(const int32_t* row_ptr, int H, int nq, int64_t* cost, cudaStream_t stream);
+constexpr int CHORUS_MAX_EXCHANGE_HEADS = 256;
+// order: HOST array of H head indices (a permutation, validated by the caller)
+cudaError_t launch_move_heads(bool scatter, const void* src, void* dst, const int32_t* order, int n_tokens,
+                              int H, int n_ranks, int row_bytes, int64_t stride_n_bytes,
+                              int64_t stride_h_bytes, cudaStream_t stream);
 void schedule_heads_host(const int64_t* cost, int H, int n_ranks, int32_t* order, int64_t* load);
 
 }  // namespace chorus
