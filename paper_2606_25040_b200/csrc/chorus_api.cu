@@ -383,6 +383,8 @@ static chorus_status move_heads(bool scatter, const void* src, void* dst, const 
         return set_error(CHORUS_ERR_INVALID_ARG, "n_tokens >= 0 and H, n_ranks, d > 0 required");
     if (H % n_ranks) return set_error(CHORUS_ERR_INVALID_ARG, "H = %d is not a multiple of n_ranks = %d", H, n_ranks);
     if (H > CHORUS_MAX_EXCHANGE_HEADS) return set_error(CHORUS_ERR_UNSUPPORTED, "H = %d > %d", H, CHORUS_MAX_EXCHANGE_HEADS);
+    if (static_cast<int64_t>(n_tokens) * H > INT32_MAX)
+        return set_error(CHORUS_ERR_CAPACITY, "n_tokens * H = %lld exceeds INT32_MAX", static_cast<long long>(n_tokens) * H);
     if (elem_bytes != 1 && elem_bytes != 2 && elem_bytes != 4)
         return set_error(CHORUS_ERR_INVALID_ARG, "elem_bytes must be 1, 2 or 4");
     const int64_t row_bytes = static_cast<int64_t>(d) * elem_bytes;
