@@ -195,7 +195,8 @@ chorus_status chorus_block_sparse_attn_fwd_first_frame(const void* Q, const void
  *   the plain decode, the flags).
  *
  * chorus_block_sparse_attn_fwd_64x128
- *   The attention call (arguments as chorus_block_sparse_attn_fwd_lse) on such an index: query row i
+ *   The attention call (arguments as chorus_block_sparse_attn_fwd_first_frame; n_first = 0 or beta = 1
+ *   for no first-frame scaling) on such an index: query row i
  *   attends the keys of the key blocks its own 64-row mask row keeps, exactly; the tiles a 128-row
  *   block's other half alone keeps are computed and masked (up to 2x the tile work of the mask when
  *   the two halves share nothing, none when they agree).  Same accuracy bounds as the plain call.
@@ -209,7 +210,7 @@ chorus_status chorus_block_sparse_attn_fwd_64x128(const void* Q, const void* K, 
                                                   float scale, chorus_dtype dtype, void* O,
                                                   const chorus_attn_shape* shape,
                                                   const chorus_fp8_scales* fp8, float* lse,
-                                                  void* cuda_stream);
+                                                  int n_first, float beta, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * FP8 quantisation pre-pass for dtype = CHORUS_FP8_E4M3 (PAPER.md:L97 says only "FP8

@@ -77,7 +77,7 @@ def lib() -> C.CDLL:
                                                        C.c_void_p, C.c_void_p]
         L.chorus_block_sparse_attn_fwd_first_frame.argtypes = (
             L.chorus_block_sparse_attn_fwd_lse.argtypes[:-1] + [C.c_int, C.c_float, C.c_void_p])
-        L.chorus_block_sparse_attn_fwd_64x128.argtypes = L.chorus_block_sparse_attn_fwd_lse.argtypes
+        L.chorus_block_sparse_attn_fwd_64x128.argtypes = L.chorus_block_sparse_attn_fwd_first_frame.argtypes
         L.chorus_mask_to_index_64x128.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                                   C.c_int64, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p]
         L.chorus_mask_from_mass.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_float, C.c_float,
@@ -222,12 +222,11 @@ def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype:
     if lse is not None:     # float32 [B][H][N], written by the kernel (natural-log row log-sum-exp)
         assert lse.dtype == torch.float32 and lse.is_contiguous() and lse.shape == (B, H, N)
     if geometry_64x128:
-        if n_first != 0 or beta != 1.0:
-            raise ChorusError(2, "first-frame scaling and the 64 x 128 geometry are not built together")
         _check(lib().chorus_block_sparse_attn_fwd_64x128(
             _ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx), C.c_float(scale), dtype, _ptr(O),
             C.byref(shape), C.byref(sc) if sc is not None else None,
-            _ptr(lse) if lse is not None else None, _stream(stream)))
+            _ptr(lse) if lse is not None else None, C.c_int(int(n_first)), C.c_float(float(beta)),
+            _stream(stream)))
         return O
     if n_first != 0 or beta != 1.0:
         _check(lib().chorus_block_sparse_attn_fwd_first_frame(

@@ -744,22 +744,16 @@ cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, cons
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
                             cudaStream_t stream) {
     const bool beta = p.n_first > 0 && p.beta != 1.f;
-    if (beta && p.half_flags) return cudaErrorNotSupported;   // not instantiated together
-    if (p.half_flags) {
-        if (dtype == CHORUS_BF16) return launch_one<false, false, false, true>(tmQ, tmK, tmV, tmO, p, stream);
-        if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, false, true>(tmQ, tmK, tmV, tmO, p, stream);
-        if (dtype == CHORUS_FP16) return launch_one<false, true, false, true>(tmQ, tmK, tmV, tmO, p, stream);
-        return cudaErrorNotSupported;
-    }
-    if (beta) {
-        if (dtype == CHORUS_BF16) return launch_one<false, false, true, false>(tmQ, tmK, tmV, tmO, p, stream);
-        if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, true, false>(tmQ, tmK, tmV, tmO, p, stream);
-        if (dtype == CHORUS_FP16) return launch_one<false, true, true, false>(tmQ, tmK, tmV, tmO, p, stream);
-        return cudaErrorNotSupported;
-    }
-    if (dtype == CHORUS_BF16) return launch_one<false, false, false, false>(tmQ, tmK, tmV, tmO, p, stream);
-    if (dtype == CHORUS_FP8_E4M3) return launch_one<true, false, false, false>(tmQ, tmK, tmV, tmO, p, stream);
-    if (dtype == CHORUS_FP16) return launch_one<false, true, false, false>(tmQ, tmK, tmV, tmO, p, stream);
+    auto go = [&](auto fp8, auto f16) -> cudaError_t {
+        constexpr bool F8 = decltype(fp8)::value, F16 = decltype(f16)::value;
+        if (beta && p.half_flags) return launch_one<F8, F16, true, true>(tmQ, tmK, tmV, tmO, p, stream);
+        if (beta) return launch_one<F8, F16, true, false>(tmQ, tmK, tmV, tmO, p, stream);
+        if (p.half_flags) return launch_one<F8, F16, false, true>(tmQ, tmK, tmV, tmO, p, stream);
+        return launch_one<F8, F16, false, false>(tmQ, tmK, tmV, tmO, p, stream);
+    };
+    if (dtype == CHORUS_BF16) return go(BoolTag<false>{}, BoolTag<false>{});
+    if (dtype == CHORUS_FP8_E4M3) return go(BoolTag<true>{}, BoolTag<false>{});
+    if (dtype == CHORUS_FP16) return go(BoolTag<false>{}, BoolTag<true>{});
     return cudaErrorNotSupported;
 }
 

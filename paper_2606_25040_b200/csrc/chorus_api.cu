@@ -234,8 +234,8 @@ chorus_status chorus_block_sparse_attn_fwd_64x128(const void* Q, const void* K, 
                                                   float scale, chorus_dtype dtype, void* O,
                                                   const chorus_attn_shape* shape,
                                                   const chorus_fp8_scales* fp8, float* lse,
-                                                  void* cuda_stream) {
-    return attn_impl(Q, K, V, row_ptr, col_idx, scale, dtype, O, shape, fp8, lse, 0, 1.0f, true, cuda_stream);
+                                                  int n_first, float beta, void* cuda_stream) {
+    return attn_impl(Q, K, V, row_ptr, col_idx, scale, dtype, O, shape, fp8, lse, n_first, beta, true, cuda_stream);
 }
 
 static chorus_status attn_impl(const void* Q, const void* K, const void* V, const int32_t* row_ptr,

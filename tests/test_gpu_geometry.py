@@ -202,3 +202,38 @@ def test_block_mass_64x128_matches_oracle_and_closes_the_loop(N, H, scale):
         gotO[t, : hi - lo] = Of[0, lo:hi, h]
     mx, mean, _, _ = err_stats(gotO, refO)
     assert mx <= BF16_MAX and mean <= BF16_MEAN, (mx, mean)
+
+
+@pytest.mark.parametrize("fp8", [False, True])
+def test_64x128_geometry_with_first_frame_scaling(fp8):
+    """Both variants at once, as the paper's pipeline uses them (L153 geometry, eq. (1) at L109-114): n_first = 330
+    straddles a 64-key tile whose key block only one half of a 128-row block may keep."""
+    N, H, n0, beta = 990, 3, 330, 1.3
+    Q, K, V, keep, bm = attention_case(N, H, seed=31)
+    rp, ci = B.chorus_mask_to_index_64x128(dmask(bm[None]), N)
+    nq64 = (N + 63) // 64
+    items = np.asarray([(0, h, qb) for h in range(H) for qb in range(nq64)], np.int32)
+    if fp8:
+        qz = B.chorus_quantize_fp8(dbf16(Q), dbf16(K), dbf16(V))
+        O = B.chorus_block_sparse_attn_fwd(qz[0], qz[1], qz[2], rp, ci, SCALE, dtype=B.CHORUS_FP8_E4M3,
+                                           fp8_scales=qz[3:], geometry_64x128=True, n_first=n0, beta=beta)
+        q8, k8, v8, qs, ks, vs = (t.cpu().numpy() for t in qz)
+        ref = oracle.block_sparse_attn(q8, k8, v8, bm, SCALE, items=items, block=(64, 128), fp8_scales=(qs, ks, vs),
+                                       n_first=n0, beta=beta)
+    else:
+        O = B.chorus_block_sparse_attn_fwd(dbf16(Q), dbf16(K), dbf16(V), rp, ci, SCALE, geometry_64x128=True,
+                                           n_first=n0, beta=beta)
+        ref = oracle.block_sparse_attn(Q, K, V, bm, SCALE, items=items, block=(64, 128), n_first=n0, beta=beta)
+    torch.cuda.synchronize()
+    Of = O.float().cpu().numpy().astype(np.float64)
+    got = np.zeros_like(ref)
+    for t, (_, h, qb) in enumerate(items):
+        lo, hi = 64 * qb, min(N, 64 * qb + 64)
+        got[t, : hi - lo] = Of[0, lo:hi, h]
+    mx, mean, _, cos = err_stats(got, ref)
+    if fp8:
+        assert mx <= FP8_MAX and cos >= FP8_COS, (mx, cos)
+    else:
+        assert mx <= BF16_MAX and mean <= BF16_MEAN, (mx, mean)
+        plain = oracle.block_sparse_attn(Q, K, V, bm, SCALE, items=items, block=(64, 128))
+        assert np.abs(plain - ref).max() > 10 * BF16_MAX          # the scaling is not a no-op here
