@@ -191,8 +191,8 @@ chorus_status chorus_block_sparse_attn_fwd_first_frame(const void* Q, const void
  *             entry  t | (upper does not keep kb) << 30 | (lower does not keep kb) << 31.
  *             An entry without flag bits is a plain chorus_mask_to_index entry.
  *   workspace as for chorus_mask_to_index (NULL = size query), 16-byte aligned.
- *   Unique result, compared bit-exactly with the oracle.  Three launches (tile mask of the row pairs,
- *   the plain decode, the flags).
+ *   Unique result, compared bit-exactly with the oracle.  One launch: the decode kernel forms the tile
+ *   mask of a row pair on the fly and never stores it.
  *
  * chorus_block_sparse_attn_fwd_64x128
  *   The attention call (arguments as chorus_block_sparse_attn_fwd_first_frame; n_first = 0 or beta = 1

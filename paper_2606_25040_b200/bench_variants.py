@@ -77,7 +77,9 @@ def main():
     for name, keep in cases:
         bm64 = torch.from_numpy(W.pack_bits(keep)[None].view(np.int32)).to(dev)
         rp64, ci64 = B.chorus_mask_to_index_64x128(bm64, N)
-        t_dec = _time(lambda: B.chorus_mask_to_index_64x128(bm64, N, row_ptr=rp64, col_idx=ci64), args.iters)
+        ws = torch.empty(1 << 20, dtype=torch.uint8, device=dev)
+        t_dec = _time(lambda: B.chorus_mask_to_index_64x128(bm64, N, row_ptr=rp64, col_idx=ci64, workspace=ws),
+                      args.iters)
         t_att = _time(lambda: B.chorus_block_sparse_attn_fwd(Q, K, V, rp64, ci64, cfg.scale, O=O,
                                                              geometry_64x128=True), args.iters)
         tiles = int(rp64[-1])

@@ -39,13 +39,51 @@ __device__ __forceinline__ unsigned long long ld_status(const unsigned long long
     return v;
 }
 
+// Source of the words when the mask is stored in the paper's 64 x 128 geometry (include/chorus.h,
+// chorus_mask_to_index_64x128): the tile mask of a 128-row block is never materialised.  Word wr of row r
+// (l, h, qb) = the union of mask rows 2 qb and 2 qb + 1, key blocks 16 wr .. 16 wr + 15, each spread over its two
+// 64-key tiles; fu / fl keep the 16 source bits of the upper / lower mask row for the per-half flags.
+struct GeoSrc {
+    const uint32_t* bm64;
+    int nq64, nq128, nk128, words128;
+};
+__device__ __forceinline__ uint32_t spread16(uint32_t x) {      // bit b of the low 16 -> bits 2b, 2b+1
+    x = (x | (x << 8)) & 0x00ff00ffu;
+    x = (x | (x << 4)) & 0x0f0f0f0fu;
+    x = (x | (x << 2)) & 0x33333333u;
+    x = (x | (x << 1)) & 0x55555555u;
+    return x | (x << 1);
+}
+__device__ __forceinline__ uint32_t geo_word(const GeoSrc& g, uint32_t r, int wr, uint32_t& fu, uint32_t& fl) {
+    const uint32_t hd = r / static_cast<uint32_t>(g.nq128), qb = r - hd * static_cast<uint32_t>(g.nq128);
+    const uint32_t* up = g.bm64 + (static_cast<int64_t>(hd) * g.nq64 + 2 * qb) * g.words128;
+    const int wi = wr >> 1, sh = 16 * (wr & 1);
+    uint32_t a = __ldg(up + wi);
+    uint32_t b = (2 * qb + 1 < static_cast<uint32_t>(g.nq64)) ? __ldg(up + g.words128 + wi) : 0u;
+    const int rem = g.nk128 - wi * 32;                          // valid key blocks of this source word
+    if (rem < 32) {
+        const uint32_t m = (1u << rem) - 1u;
+        a &= m;
+        b &= m;
+    }
+    fu = (a >> sh) & 0xffffu;
+    fl = (b >> sh) & 0xffffu;
+    return spread16(fu | fl);
+}
+// entry of tile bit b (tile index t): t | upper half does not keep it << 30 | lower half does not << 31
+__device__ __forceinline__ int32_t geo_entry(int t, int b, uint32_t fu, uint32_t fl) {
+    const uint32_t nu = (~fu >> (b >> 1)) & 1u, nl = (~fl >> (b >> 1)) & 1u;
+    return static_cast<int32_t>(static_cast<uint32_t>(t) | (nu << 30) | (nl << 31));
+}
+
 // WPT consecutive words per thread: 4 for large mask sets (fewer scans, divisions and status words per
 // word), 1 for a single layer (more, smaller tiles: one 480p layer is only 160 K words)
-template <int WPT>
+template <int WPT, bool kGeo>
 __global__ void __launch_bounds__(DEC_THREADS)
 decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, int words,
                     int32_t* __restrict__ row_ptr, int32_t* __restrict__ col_idx, int64_t col_cap,
-                    unsigned long long* __restrict__ status /* [0] = ticket counter, [1 + t] = tile t */) {
+                    unsigned long long* __restrict__ status /* [0] = ticket counter, [1 + t] = tile t */,
+                    const GeoSrc geo) {
     // entry e sits at e + e/32: threads whose runs start 8, 16 or 32 entries apart (25 %, 50 %, full
     // density) then hit different banks when they all write their k-th entry
     __shared__ int32_t s_stage[STAGE + STAGE / 32];
@@ -66,18 +104,26 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
     // 1. load WPT consecutive words per thread, mask the pad bits, count
     const uint32_t w0 = tile0 + threadIdx.x * WPT;              // this thread's first word
     uint32_t v[WPT];
+    uint32_t fu[kGeo ? WPT : 1], fl[kGeo ? WPT : 1];            // kGeo: source bits of the two mask rows
     const uint32_t row0 = w0 / static_cast<uint32_t>(words);    // one division per thread and tile
     const int win0 = static_cast<int>(w0 - row0 * static_cast<uint32_t>(words));
     int cnt = 0;
     {
         int wr = win0;
+        uint32_t r = row0;
 #pragma unroll
         for (int i = 0; i < WPT; ++i) {
-            uint32_t x = (w0 + i < n_words) ? __ldg(bitmask + w0 + i) : 0u;
+            uint32_t x = 0u;
+            if constexpr (kGeo) {
+                fu[i] = fl[i] = 0u;
+                if (w0 + i < n_words) x = geo_word(geo, r, wr, fu[i], fl[i]);
+            } else {
+                if (w0 + i < n_words) x = __ldg(bitmask + w0 + i);
+            }
             if (wr == words - 1) x &= last_mask;
             v[i] = x;
             cnt += __popc(x);
-            if (++wr == words) wr = 0;
+            if (++wr == words) { wr = 0; ++r; }
         }
     }
     // 2a/2b. one exclusive scan of the thread counts inside the block
@@ -114,7 +160,7 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
                 while (x) {
                     const int b = __ffs(x) - 1;
                     x &= x - 1;
-                    s_stage[e + (e >> 5)] = kb0 + b;
+                    s_stage[e + (e >> 5)] = kGeo ? geo_entry(kb0 + b, b, fu[i], fl[i]) : kb0 + b;
                     ++e;
                 }
                 if (++wr == words) wr = 0;
@@ -191,15 +237,17 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
             const int lo = s_woff[r * DEC_THREADS];
             const int hi = r + 1 < WPT ? s_woff[(r + 1) * DEC_THREADS] : tile_total;
             const uint32_t g = tile0 + j;
-            const int wr = static_cast<int>(g % static_cast<uint32_t>(words));
-            uint32_t x = g < n_words ? __ldg(bitmask + g) : 0u;
+            const uint32_t gr = g / static_cast<uint32_t>(words);
+            const int wr = static_cast<int>(g - gr * static_cast<uint32_t>(words));
+            uint32_t x = 0u, gu = 0u, gl = 0u;
+            if (g < n_words) x = kGeo ? geo_word(geo, gr, wr, gu, gl) : __ldg(bitmask + g);
             if (wr == words - 1) x &= last_mask;
             int e = s_woff[j] - lo;
             const int kb0 = wr * 32;
             while (x) {
                 const int b = __ffs(x) - 1;
                 x &= x - 1;
-                s_stage[e + (e >> 5)] = kb0 + b;
+                s_stage[e + (e >> 5)] = kGeo ? geo_entry(kb0 + b, b, gu, gl) : kb0 + b;
                 ++e;
             }
             __syncthreads();
@@ -229,57 +277,6 @@ visit_refresh_kernel(uint32_t* __restrict__ bitmask, int n_groups, int64_t words
 }
 
 // one word per thread below this many words (a few layers), four above
-// ---- masks in the paper's 64 x 128 geometry (include/chorus.h) ---------------------
-// Step 1: the 64-key-tile mask of every 128-row block = union of its two 64-row mask rows, each key
-// block (128 keys) spread over its two tiles.  One thread per output word.
-__device__ __forceinline__ uint32_t spread16(uint32_t x) {      // bit b of the low 16 -> bits 2b, 2b+1
-    x = (x | (x << 8)) & 0x00ff00ffu;
-    x = (x | (x << 4)) & 0x0f0f0f0fu;
-    x = (x | (x << 2)) & 0x33333333u;
-    x = (x | (x << 1)) & 0x55555555u;
-    return x | (x << 1);
-}
-__global__ void __launch_bounds__(256)
-union_tiles_kernel(const uint32_t* __restrict__ bm64, int64_t heads /* L*H */, int nq64, int nq128,
-                   int nk128, int words128, int words64, uint32_t* __restrict__ out) {
-    const int64_t total = heads * nq128 * words64;
-    for (int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < total;
-         i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
-        const int wo = static_cast<int>(i % words64);
-        const int64_t R = i / words64;
-        const int qb = static_cast<int>(R % nq128);
-        const int64_t hd = R / nq128;
-        const int wi = wo >> 1;
-        const uint32_t* up = bm64 + (hd * nq64 + 2 * qb) * words128;
-        uint32_t u = up[wi];
-        if (2 * qb + 1 < nq64) u |= up[words128 + wi];
-        const int rem = nk128 - wi * 32;                        // valid key blocks of this word
-        if (rem < 32) u &= (1u << rem) - 1u;
-        out[i] = spread16((u >> (16 * (wo & 1))) & 0xffffu);
-    }
-}
-
-// Step 3 (step 2 is the plain decode of that mask): one warp per 128-row block marks, in every entry,
-// which of its two halves does NOT keep the tile's key block.
-__global__ void __launch_bounds__(256)
-half_flags_kernel(const uint32_t* __restrict__ bm64, int64_t rows128, int nq64, int nq128, int words128,
-                  const int32_t* __restrict__ row_ptr, int32_t* __restrict__ col_idx, int64_t col_cap) {
-    const int64_t R = (static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
-    if (R >= rows128) return;
-    const int lane = threadIdx.x & 31;
-    const int qb = static_cast<int>(R % nq128);
-    const int64_t hd = R / nq128;
-    const uint32_t* up = bm64 + (hd * nq64 + 2 * qb) * words128;
-    const bool has_lo = 2 * qb + 1 < nq64;
-    const int64_t e1 = min(static_cast<int64_t>(row_ptr[R + 1]), col_cap);
-    for (int64_t e = row_ptr[R] + lane; e < e1; e += 32) {
-        const int t = col_idx[e], kb = t >> 1;
-        const uint32_t ku = (up[kb >> 5] >> (kb & 31)) & 1u;
-        const uint32_t kl = has_lo ? (up[words128 + (kb >> 5)] >> (kb & 31)) & 1u : 0u;
-        col_idx[e] = static_cast<int32_t>(static_cast<uint32_t>(t) | ((ku ^ 1u) << 30) | ((kl ^ 1u) << 31));
-    }
-}
-
 constexpr int64_t SMALL_WORDS = 1 << 20;
 inline int wpt_for(int64_t n_words) { return n_words < SMALL_WORDS ? 1 : 4; }
 inline int64_t n_tiles_for(int64_t rows, int words) {
@@ -294,21 +291,31 @@ size_t decode_workspace_bytes(int64_t rows, int words) {
     return static_cast<size_t>(n_tiles_for(rows, words) + 1) * sizeof(unsigned long long) + 8;
 }
 
-cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, int words,
-                               int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
-                               cudaStream_t stream) {
+static cudaError_t launch_decode(const uint32_t* bitmask, const GeoSrc* geo, int64_t rows, int nk, int words,
+                                 int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
+                                 cudaStream_t stream) {
     const int64_t nt = n_tiles_for(rows, words);
     auto* status = reinterpret_cast<unsigned long long*>((reinterpret_cast<uintptr_t>(workspace) + 7) & ~uintptr_t(7));
     cudaError_t e = cudaMemsetAsync(status, 0, static_cast<size_t>(nt + 1) * sizeof(unsigned long long), stream);
     if (e != cudaSuccess) return e;
-    if (wpt_for(rows * words) == 1)
-        decode_tiles_kernel<1><<<static_cast<unsigned>(nt), DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr,
-                                                                                    col_idx, col_cap, status);
-    else
-        decode_tiles_kernel<4><<<static_cast<unsigned>(nt), DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr,
-                                                                                    col_idx, col_cap, status);
+    const unsigned grid = static_cast<unsigned>(nt);
+    const bool one = wpt_for(rows * words) == 1;
+    const GeoSrc g = geo ? *geo : GeoSrc{nullptr, 0, 0, 0, 0};
+    if (geo) {
+        if (one) decode_tiles_kernel<1, true><<<grid, DEC_THREADS, 0, stream>>>(nullptr, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+        else decode_tiles_kernel<4, true><<<grid, DEC_THREADS, 0, stream>>>(nullptr, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+    } else {
+        if (one) decode_tiles_kernel<1, false><<<grid, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+        else decode_tiles_kernel<4, false><<<grid, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+    }
     count_launch(1);
     return cudaGetLastError();
+}
+
+cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, int words,
+                               int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
+                               cudaStream_t stream) {
+    return launch_decode(bitmask, nullptr, rows, nk, words, row_ptr, col_idx, col_cap, workspace, stream);
 }
 
 cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_layer, int words,
@@ -325,30 +332,16 @@ cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_lay
 
 size_t decode_64x128_workspace_bytes(int64_t heads, int N) {
     const int nq128 = (N + 127) / 128, words64 = ((N + 63) / 64 + 31) / 32;
-    const size_t un = (static_cast<size_t>(heads) * nq128 * words64 * 4 + 15) & ~size_t(15);
-    return un + decode_workspace_bytes(heads * nq128, words64);
+    return decode_workspace_bytes(heads * nq128, words64);
 }
 
+// One launch: the decode kernel reads the 64 x 128 mask rows directly (GeoSrc) and writes the flagged entries.
 cudaError_t launch_mask_decode_64x128(const uint32_t* bm64, int64_t heads, int N, int32_t* row_ptr,
                                       int32_t* col_idx, int64_t col_cap, void* workspace, cudaStream_t stream) {
     const int nq64 = (N + 63) / 64, nq128 = (N + 127) / 128, nk128 = nq128, nk64 = nq64;
-    const int words128 = (nk128 + 31) / 32, words64 = (nk64 + 31) / 32;
-    const int64_t rows128 = heads * nq128;
-    uint32_t* un = static_cast<uint32_t*>(workspace);
-    const size_t un_bytes = (static_cast<size_t>(rows128) * words64 * 4 + 15) & ~size_t(15);
-    const int64_t total = rows128 * words64;
-    const int blocks = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 16));
-    union_tiles_kernel<<<blocks, 256, 0, stream>>>(bm64, heads, nq64, nq128, nk128, words128, words64, un);
-    count_launch(1);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    e = launch_mask_decode(un, rows128, nk64, words64, row_ptr, col_idx, col_cap,
-                           static_cast<char*>(workspace) + un_bytes, stream);
-    if (e != cudaSuccess || col_idx == nullptr) return e;
-    half_flags_kernel<<<static_cast<unsigned>((rows128 * 32 + 255) / 256), 256, 0, stream>>>(
-        bm64, rows128, nq64, nq128, words128, row_ptr, col_idx, col_cap);
-    count_launch(1);
-    return cudaGetLastError();
+    const GeoSrc geo{bm64, nq64, nq128, nk128, (nk128 + 31) / 32};
+    return launch_decode(nullptr, &geo, heads * nq128, nk64, (nk64 + 31) / 32, row_ptr, col_idx, col_cap,
+                         workspace, stream);
 }
 
 }  // namespace chorus

@@ -25,7 +25,8 @@ def random_mask(L, H, N, rho, seed):
 
 
 @pytest.mark.parametrize("L,H,N,rho", [(1, 1, 64, 1.0), (2, 3, 65, 0.5), (1, 2, 129, 0.5), (2, 2, 4200, 0.3),
-                                       (1, 3, 8256, 0.1), (3, 2, 2049, 0.7), (1, 40, 32760, 0.25)])
+                                       (1, 3, 8256, 0.1), (3, 2, 2049, 0.7), (1, 40, 32760, 0.25),
+                                       (8, 40, 32760, 0.12), (7, 40, 32767, 0.6)])   # >= 2^20 tile-mask words: 4 per thread
 def test_decode_64x128_bit_exact(L, H, N, rho):
     keep, bm = random_mask(L, H, N, rho, seed=N + L)
     rp_o, ci_o = oracle.mask_to_index_64x128(bm, N)
