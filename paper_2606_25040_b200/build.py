@@ -52,7 +52,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if failed:
         raise RuntimeError("nvcc failed")
     tmp = LIB + f".tmp{os.getpid()}"
-    subprocess.run([NVCC, "-shared", "-o", tmp, *objs, "-lcudart"], check=True)
+    subprocess.run([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs, "-lcudart"],
+                   check=True)
     os.replace(tmp, LIB)
     return LIB
 
