@@ -31,8 +31,9 @@
  *     and the call returns without synchronising.
  *   - Errors: an integer status, never an exception.  Argument errors are detected on the host
  *     before anything is launched.  chorus_last_error() gives a thread-local message.
- *   - Block geometry is fixed: 128 query rows x 64 keys per block, head_dim 128
- *     (BASELINE.json north_star; the paper's own run used 64 x 128).
+ *   - The kernels' tile is fixed: 128 query rows x 64 keys, head_dim 128 (BASELINE.json north_star).
+ *     Masks in the paper's own 64 x 128 block geometry go through the *_64x128
+ *     entry points, which serve them exactly on the same tiles.
  *   - There is no CPU fallback: without a CUDA device every compute entry point returns
  *     CHORUS_ERR_CUDA.
  */
@@ -132,7 +133,8 @@ typedef struct {
  *           nq_blk = ceil(N/128); the same mask is used for every b.
  * col_idx   device, the base pointer that row_ptr's absolute offsets index into.  Indices must
  *           lie in [0, ceil(N/64)) and ascend within a row (what chorus_mask_to_index produces);
- *           anything else is undefined behaviour.
+ *           anything else is undefined behaviour (an index with the per-half flag bits of
+ *           chorus_mask_to_index_64x128 belongs to chorus_block_sparse_attn_fwd_64x128 only).
  * scale     multiplies QK^T before the softmax (1/sqrt(128) in all workloads).
  * O         device, bf16 for dtype BF16 and FP8_E4M3, fp16 for dtype FP16; 16-byte aligned, strides
  *           multiples of 8 elements.
