@@ -55,9 +55,11 @@ def heads_to_seq(o_heads, order, group=None, out=None, _scatter=None):
     return out
 
 
-def rank_row_ptr(row_ptr, order, rank: int, n_ranks: int, nq_blk: int):
-    """Rows of this rank's heads, in schedule order, as (head, first row, last row + 1) triples into the
-    layer's row_ptr: the attention call takes one head (or one run of consecutive heads) at a time."""
+def rank_rows(order, rank: int, n_ranks: int, nq_blk: int):
+    """This rank's heads in schedule order as (head, first row, last row + 1) triples into the layer's row_ptr
+    (rows of head h are h * nq_blk .. (h + 1) * nq_blk).  After seq_to_heads the rank's tensors hold these heads
+    in this order, so either the mask rows are gathered the same way before the decode (the masks follow their
+    heads) or the attention call is made per head with row_ptr[first : last + 1]."""
     H = len(order)
     slots = H // n_ranks
     return [(int(h), int(h) * nq_blk, (int(h) + 1) * nq_blk) for h in order[rank * slots:(rank + 1) * slots]]

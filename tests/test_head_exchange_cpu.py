@@ -55,7 +55,7 @@ def _worker(rank, world, port, q):
         back = ulysses.heads_to_seq(oh.contiguous(), order, _scatter=scatter)
         ref = (X * 2.0 + np.arange(N, dtype=np.float32)[:, None, None])[rank * n_loc:(rank + 1) * n_loc]
         ok2 = back.shape == (1, n_loc, H, d) and np.array_equal(back[0].numpy(), ref)
-        rows = ulysses.rank_row_ptr(None, order, rank, world, nq_blk=5)
+        rows = ulysses.rank_rows(order, rank, world, nq_blk=5)
         ok3 = rows == [(h, 5 * h, 5 * h + 5) for h in mine]
         q.put((rank, bool(ok1), bool(ok2), bool(ok3)))
     finally:
