@@ -124,3 +124,17 @@ def test_block_mass_64x128_equals_numpy_softmax_summed_per_block():
     a = m[0, :, : 2 * (nq64 // 2)].reshape(H, nq64 // 2, 2, nk128).sum(axis=2)
     b = np.pad(m2[0], ((0, 0), (0, 0), (0, 2 * nk128 - m2.shape[3]))).reshape(H, m2.shape[2], nk128, 2).sum(axis=3)
     np.testing.assert_allclose(a, b[:, : nq64 // 2], rtol=0, atol=1e-12)
+
+
+def test_decode_64x128_golden_hand_worked_example():
+    """tests/golden/decode_64x128.txt: derived by hand from the definition (R26), not by any program."""
+    import os
+    vals = {}
+    for line in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "decode_64x128.txt")):
+        if not line.startswith("#") and line.strip():
+            k, *v = line.split()
+            vals[k] = [int(x) for x in v]
+    N = vals["N"][0]
+    bm = np.array(vals["mask_rows"], np.uint32).reshape(1, 1, 4, 1)       # one word per mask row: bit kb
+    rp, ci = oracle.mask_to_index_64x128(bm, N)
+    assert rp.tolist() == vals["row_ptr"] and ci.tolist() == vals["col_idx"]
