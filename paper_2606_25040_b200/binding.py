@@ -12,7 +12,7 @@ import os
 import torch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libchorus.so")
+LIB_PATH = os.environ.get("CHORUS_LIB") or os.path.join(HERE, "libchorus.so")   # CHORUS_LIB: another build of the library
 
 CHORUS_OK, CHORUS_ERR_INVALID_ARG, CHORUS_ERR_UNSUPPORTED, CHORUS_ERR_CAPACITY, CHORUS_ERR_CUDA = range(5)
 CHORUS_BF16, CHORUS_FP8_E4M3, CHORUS_FP16 = 0, 1, 2

@@ -55,7 +55,10 @@ using namespace ptx;
 #define PHASE_MARK(i) do { } while (0)
 #endif
 #ifndef CHORUS_POLY_MASK
-#define CHORUS_POLY_MASK 0x00u   // e.g. 0x4A = 3 of every 8 element pairs
+#define CHORUS_POLY_MASK 0x00u       // bf16 / fp16: every exponential on the MUFU (a polynomial share was never faster)
+#endif
+#ifndef CHORUS_POLY_MASK_FP8
+#define CHORUS_POLY_MASK_FP8 0x11u   // fp8: 2 of every 8 element pairs on the FMA pipe (2-3 % faster, profiles/r01_v5.md)
 #endif
 constexpr int BQ = 128, BK = 64;
 constexpr int SBUFS = 3;
@@ -92,7 +95,7 @@ struct Cfg {
     static constexpr float P_SHIFT = kFp8 ? 5.0f : 0.0f;
     // which element pairs (index mod 8) take the FMA-pipe polynomial exp2 instead of the MUFU, and
     // its degree (relative error 7.5e-5 / 1.7e-3, below the bf16 / e4m3 rounding of P)
-    static constexpr uint32_t POLY_MASK = CHORUS_POLY_MASK;
+    static constexpr uint32_t POLY_MASK = kFp8 ? CHORUS_POLY_MASK_FP8 : CHORUS_POLY_MASK;
     static constexpr int POLY_DEG = kFp8 ? 2 : 3;
     // TMEM columns of P per MMA step (16 bf16 keys or 32 e4m3 keys = 8 columns), steps per tile
     static constexpr int PV_STEPS_PER_TILE = kFp8 ? 2 : 4;
