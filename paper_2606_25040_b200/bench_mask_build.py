@@ -50,10 +50,12 @@ def main():
     rp, ci = B.chorus_mask_to_index(full, cfg.nk)
     lse = torch.empty((1, cfg.H, cfg.N), dtype=torch.float32, device=dev)
     O = torch.empty_like(Q)
-    t_attn = _time(lambda: B.chorus_block_sparse_attn_fwd(Q, K, V, rp, ci, cfg.scale, O=O, lse=lse), args.iters)
     mass = torch.empty((1, cfg.H, cfg.nq, cfg.nk), dtype=torch.float32, device=dev)
-    t2 = _time(lambda: B.chorus_block_mass(Q, K, cfg.scale, mass=mass), args.iters)
-    t1 = _time(lambda: B.chorus_block_mass(Q, K, cfg.scale, mass=mass, lse=lse), args.iters)
+    # two rounds, the second one reported: the first kernels of a process run at boost clocks
+    for _ in range(2):
+        t_attn = _time(lambda: B.chorus_block_sparse_attn_fwd(Q, K, V, rp, ci, cfg.scale, O=O, lse=lse), args.iters)
+        t2 = _time(lambda: B.chorus_block_mass(Q, K, cfg.scale, mass=mass), args.iters)
+        t1 = _time(lambda: B.chorus_block_mass(Q, K, cfg.scale, mass=mass, lse=lse), args.iters)
     bm = torch.empty((cfg.H, cfg.nq, cfg.words), dtype=torch.int32, device=dev)
     kept = torch.empty((cfg.H, cfg.nq), dtype=torch.int32, device=dev)
     t_sel = _time(lambda: B.chorus_mask_from_mass(mass[0], 0.9, 0.1, bitmask=bm, kept=kept), args.iters)
