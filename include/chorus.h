@@ -135,7 +135,9 @@ typedef struct {
  *           lie in [0, ceil(N/64)) and ascend within a row (what chorus_mask_to_index produces);
  *           anything else is undefined behaviour (an index with the per-half flag bits of
  *           chorus_mask_to_index_64x128 belongs to chorus_block_sparse_attn_fwd_64x128 only).
- * scale     multiplies QK^T before the softmax (1/sqrt(128) in all workloads).
+ * scale     multiplies QK^T before the softmax (1/sqrt(128) in all workloads).  Must be positive and
+ *           finite (the row maximum is taken on the raw scores): anything else is INVALID_ARG, here
+ *           and in chorus_block_mass.
  * O         device, bf16 for dtype BF16 and FP8_E4M3, fp16 for dtype FP16; 16-byte aligned, strides
  *           multiples of 8 elements.
  * fp8       non-NULL iff dtype == CHORUS_FP8_E4M3.
@@ -291,8 +293,8 @@ chorus_status chorus_block_mass(const void* Q, const void* K, float scale,
 chorus_status chorus_block_mass_64x128(const void* Q, const void* K, float scale,
                                        const chorus_attn_shape* shape, const float* lse, float* mass,
                                        void* cuda_stream);
-chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk, float top_p,
-                                    float min_top_k, uint32_t* bitmask, int32_t* kept,
+chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk, double top_p,
+                                    double min_top_k, uint32_t* bitmask, int32_t* kept,
                                     void* cuda_stream);
 chorus_status chorus_mask_coverage(const float* mass, const uint32_t* bitmask, int heads, int nq_blk,
                                    int nk_blk, float* coverage, void* cuda_stream);

@@ -12,7 +12,7 @@ import os
 import torch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("CHORUS_LIB") or os.path.join(HERE, "libchorus.so")   # CHORUS_LIB: another build of the library
+LIB_PATH = os.path.join(HERE, "libchorus.so")
 
 CHORUS_OK, CHORUS_ERR_INVALID_ARG, CHORUS_ERR_UNSUPPORTED, CHORUS_ERR_CAPACITY, CHORUS_ERR_CUDA = range(5)
 CHORUS_BF16, CHORUS_FP8_E4M3, CHORUS_FP16 = 0, 1, 2
@@ -80,7 +80,7 @@ def lib() -> C.CDLL:
         L.chorus_block_sparse_attn_fwd_64x128.argtypes = L.chorus_block_sparse_attn_fwd_first_frame.argtypes
         L.chorus_mask_to_index_64x128.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                                   C.c_int64, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p]
-        L.chorus_mask_from_mass.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_float, C.c_float,
+        L.chorus_mask_from_mass.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double,
                                             C.c_void_p, C.c_void_p, C.c_void_p]
         L.chorus_mask_coverage.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
                                            C.c_void_p, C.c_void_p]
@@ -315,7 +315,7 @@ def chorus_mask_from_mass(mass, top_p: float, min_top_k: float, bitmask=None, ke
         bitmask = torch.empty(mass.shape[:-1] + ((nk + 31) // 32,), dtype=torch.int32, device=mass.device)
     if kept is None:
         kept = torch.empty(mass.shape[:-1], dtype=torch.int32, device=mass.device)
-    _check(lib().chorus_mask_from_mass(_ptr(mass), rows, nk, C.c_float(top_p), C.c_float(min_top_k),
+    _check(lib().chorus_mask_from_mass(_ptr(mass), rows, nk, C.c_double(top_p), C.c_double(min_top_k),
                                        _ptr(bitmask), _ptr(kept), _stream(stream)))
     return bitmask, kept
 

@@ -19,8 +19,6 @@ HEADERS = ["chorus_internal.h", "sm100_ptx.cuh", os.path.join("..", "..", "inclu
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
          "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall"]
-# extra nvcc flags for tuning sweeps, e.g. CHORUS_NVCC_FLAGS="-DCHORUS_POLY_MASK=0x5Au"
-FLAGS += os.environ.get("CHORUS_NVCC_FLAGS", "").split()
 
 
 def _stale() -> bool:

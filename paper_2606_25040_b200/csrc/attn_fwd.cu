@@ -32,8 +32,6 @@
 // 64-key tile and V's per-channel scale applied in the epilogue.
 #include <cuda_bf16.h>
 
-#include <cstdio>
-
 #include "chorus_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -42,24 +40,6 @@ namespace {
 
 using namespace ptx;
 
-#ifndef CHORUS_EXP_TOKEN
-#define CHORUS_EXP_TOKEN 0
-#endif
-// debug only: per-phase cycle counters of the softmax warps of CTA 0, printed at kernel exit
-#ifndef CHORUS_PHASE_CLOCKS
-#define CHORUS_PHASE_CLOCKS 0
-#endif
-#if CHORUS_PHASE_CLOCKS
-#define PHASE_MARK(i) do { const long long t_ = clock64(); ph_acc[i] += t_ - ph_t; ph_t = t_; } while (0)
-#else
-#define PHASE_MARK(i) do { } while (0)
-#endif
-#ifndef CHORUS_POLY_MASK
-#define CHORUS_POLY_MASK 0x00u       // bf16 / fp16: every exponential on the MUFU (a polynomial share was never faster)
-#endif
-#ifndef CHORUS_POLY_MASK_FP8
-#define CHORUS_POLY_MASK_FP8 0x11u   // fp8: 2 of every 8 element pairs on the FMA pipe (2-3 % faster, profiles/r01_v5.md)
-#endif
 constexpr int BQ = 128, BK = 64;
 constexpr int SBUFS = 3;
 constexpr int NUM_THREADS = 384;
@@ -95,7 +75,7 @@ struct Cfg {
     static constexpr float P_SHIFT = kFp8 ? 5.0f : 0.0f;
     // which element pairs (index mod 8) take the FMA-pipe polynomial exp2 instead of the MUFU, and
     // its degree (relative error 7.5e-5 / 1.7e-3, below the bf16 / e4m3 rounding of P)
-    static constexpr uint32_t POLY_MASK = kFp8 ? CHORUS_POLY_MASK_FP8 : CHORUS_POLY_MASK;
+    static constexpr uint32_t POLY_MASK = kFp8 ? 0x11u : 0x00u;   // fp8: 2 of every 8 pairs; bf16 / fp16: none (never faster)
     static constexpr int POLY_DEG = kFp8 ? 2 : 3;
     // TMEM columns of P per MMA step (16 bf16 keys or 32 e4m3 keys = 8 columns), steps per tile
     static constexpr int PV_STEPS_PER_TILE = kFp8 ? 2 : 4;
@@ -359,11 +339,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         volatile float* xe = xch + 128;          // [2 parity][m, l][128] epilogue exchange
         uint32_t g0 = 0;                         // pairs of all previous items (S buffer / phase)
         uint32_t icnt = 0;                       // non-empty items so far
-#if CHORUS_PHASE_CLOCKS
-        long long ph_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, ph_t = clock64();
-        const long long ph_t0 = ph_t;
-        int ph_pairs = 0;
-#endif
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
             const Item it = get_item(p, idx);
             float m_ref = -INFINITY, l0 = 0.f, l1 = 0.f;
@@ -428,10 +403,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     if (skip_a) va = 0;
                     if (skip_b) vb = 0;
                 }
-                PHASE_MARK(0);
                 mbar_wait(bar(C::B_S_FULL + sb), (g / SBUFS) & 1);
                 tc_fence_after();
-                PHASE_MARK(1);
                 // The 128 scores of a row are streamed from tensor memory twice, 32 columns at a time
                 // with the next chunk's load in flight (pass 1: row max; pass 2: exp, pack, store P
                 // behind the read position), so that only 64 of them are ever live in registers.
@@ -483,7 +456,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     mxb = fmaxf(mxb, max32(rb));
                 }
                 const float mt = fmaxf(mxa * sl2a, mxb * sl2b);   // sl2 > 0; va > 0
-                PHASE_MARK(2);
                 // m_ref hand-off: the other parity published the reference it used for pair j - 1
                 // (and under which O now stands) after ITS max pass.
                 if (j > 0) {
@@ -507,11 +479,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 }
                 if (j + 1 < it.np) {                 // publish before the (rare) rescale: P V of pair j + 1
                     xm[row] = m_ref;                 // cannot be issued before this pair's P is ready
-#if !CHORUS_EXP_TOKEN
                     named_bar_arrive(NB_HAND + sm * 4 + wq, 64);
-#endif
                 }
-                PHASE_MARK(3);
                 if (grow && j > 0) {
                     // O holds pairs 0..j-1 under the old reference; wait for P V of pair j-1.
                     // (S_FULL of pair g implies P V of pair g-3 is complete, so the barrier of
@@ -588,12 +557,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     l0 = lacc.x;
                     l1 = lacc.y;
                 }
-#if CHORUS_EXP_TOKEN
-                // The hand-off doubles as an exp-phase token: the other parity starts its exp pass
-                // only now, so the two warps of a sub-partition never compete for the MUFU and one
-                // of them is always in its (MUFU-free) load / max phase.
-                if (j + 1 < it.np) named_bar_arrive(NB_HAND + sm * 4 + wq, 64);
-#endif
                 };
                 // kHalf: the rows of this warp keep neither tile of the pair (the other half of the block
                 // does): no pass over S, P = 0, the reference is handed on unchanged
@@ -621,17 +584,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 if (kHalf && va == 0 && vb == 0) skip_body();
                 else if (ragged) pair_body(BoolTag<true>{});
                 else pair_body(BoolTag<false>{});
-                PHASE_MARK(4);
                 tc_wait_st();
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(C::B_P_READY + sb));
-                PHASE_MARK(5);
-#if CHORUS_PHASE_CLOCKS
-                ++ph_pairs;
-#endif
             }
-            PHASE_MARK(0);
             g0 += it.np;
             // ---------------- epilogue: add the partial row sums, normalise, convert, store ------
             // Warp (sm, wq) finalises O columns [64 sm, 64 sm + 64) of its 32 rows.  The parity that
@@ -711,14 +668,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             }
         }
         if (lane == 0 && wq == 0) tma_store_wait_all();
-#if CHORUS_PHASE_CLOCKS
-        PHASE_MARK(6);
-        if (blockIdx.x == 0 && lane == 0 && wq == 1)
-            printf("phase clocks warp %d: pairs %d total %lld | per pair: top %lld waitS %lld max %lld hand %lld exp %lld "
-                   "st+arrive %lld | epilogue total %lld\n", warp, ph_pairs, clock64() - ph_t0, ph_acc[0] / ph_pairs,
-                   ph_acc[1] / ph_pairs, ph_acc[2] / ph_pairs, ph_acc[3] / ph_pairs, ph_acc[4] / ph_pairs,
-                   ph_acc[5] / ph_pairs, ph_acc[6]);
-#endif
     }
     tc_fence_before();
     __syncthreads();

@@ -243,6 +243,8 @@ static chorus_status attn_impl(const void* Q, const void* K, const void* V, cons
                                const chorus_attn_shape* shape, const chorus_fp8_scales* fp8, float* lse,
                                int n_first, float beta, bool half_flags, void* cuda_stream) {
     g_err[0] = 0;
+    if (!(scale > 0.f) || !(scale <= 3.0e38f))
+        return set_error(CHORUS_ERR_INVALID_ARG, "scale = %g must be positive and finite", static_cast<double>(scale));
     if (n_first < 0) return set_error(CHORUS_ERR_INVALID_ARG, "n_first = %d is negative", n_first);
     if (!(beta > 0.f) || !(beta <= 3.0e38f))
         return set_error(CHORUS_ERR_INVALID_ARG, "beta = %g must be positive and finite", static_cast<double>(beta));
@@ -312,6 +314,8 @@ chorus_status chorus_block_mass_64x128(const void* Q, const void* K, float scale
 static chorus_status block_mass_impl(const void* Q, const void* K, float scale, const chorus_attn_shape* shape,
                                      const float* lse, float* mass, bool geo64, void* cuda_stream) {
     g_err[0] = 0;
+    if (!(scale > 0.f) || !(scale <= 3.0e38f))
+        return set_error(CHORUS_ERR_INVALID_ARG, "scale = %g must be positive and finite", static_cast<double>(scale));
     if (!Q || !K || !mass) return set_error(CHORUS_ERR_INVALID_ARG, "Q, K, mass must be non-null");
     if (!aligned16(Q) || !aligned16(K)) return set_error(CHORUS_ERR_INVALID_ARG, "Q, K must be 16-byte aligned");
     if (!shape) return set_error(CHORUS_ERR_INVALID_ARG, "shape is null");
@@ -329,18 +333,17 @@ static chorus_status block_mass_impl(const void* Q, const void* K, float scale, 
                                         static_cast<cudaStream_t>(cuda_stream)), "block mass launch");
 }
 
-chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk, float top_p,
-                                    float min_top_k, uint32_t* bitmask, int32_t* kept,
+chorus_status chorus_mask_from_mass(const float* mass, int64_t rows, int nk_blk, double top_p,
+                                    double min_top_k, uint32_t* bitmask, int32_t* kept,
                                     void* cuda_stream) {
     g_err[0] = 0;
     if (!mass || !bitmask) return set_error(CHORUS_ERR_INVALID_ARG, "mass / bitmask is null");
     if (rows <= 0 || nk_blk <= 0) return set_error(CHORUS_ERR_INVALID_ARG, "rows, nk_blk must be positive");
     if (rows > INT32_MAX) return set_error(CHORUS_ERR_CAPACITY, "rows = %lld exceeds INT32_MAX", (long long)rows);
     if (nk_blk > 2048) return set_error(CHORUS_ERR_UNSUPPORTED, "nk_blk = %d > 2048", nk_blk);
-    if (!(top_p >= 0.f && top_p <= 1.f) || !(min_top_k >= 0.f && min_top_k <= 1.f))
+    if (!(top_p >= 0.0 && top_p <= 1.0) || !(min_top_k >= 0.0 && min_top_k <= 1.0))
         return set_error(CHORUS_ERR_INVALID_ARG, "top_p and min_top_k must lie in [0, 1]");
-    return check_cuda(launch_mask_from_mass(mass, rows, nk_blk, static_cast<double>(top_p),
-                                            static_cast<double>(min_top_k), bitmask, kept,
+    return check_cuda(launch_mask_from_mass(mass, rows, nk_blk, top_p, min_top_k, bitmask, kept,
                                             static_cast<cudaStream_t>(cuda_stream)), "mask_from_mass launch");
 }
 

@@ -73,10 +73,10 @@ def test_argument_validation_on_host(lib):
     assert lib.chorus_block_mass(None, fake, C.c_float(1.0), C.byref(shp), None, fake, None) == B.CHORUS_ERR_INVALID_ARG
     shp64 = B.AttnShape(B=1, H=1, N=128, d=64)
     assert lib.chorus_block_mass(fake, fake, C.c_float(1.0), C.byref(shp64), None, fake, None) == B.CHORUS_ERR_UNSUPPORTED
-    assert lib.chorus_mask_from_mass(fake, 4, 4096, C.c_float(0.9), C.c_float(0.1), fake, None, None) == B.CHORUS_ERR_UNSUPPORTED
-    assert lib.chorus_mask_from_mass(fake, 4, 64, C.c_float(1.5), C.c_float(0.1), fake, None, None) == B.CHORUS_ERR_INVALID_ARG
-    assert lib.chorus_mask_from_mass(fake, 0, 64, C.c_float(0.9), C.c_float(0.1), fake, None, None) == B.CHORUS_ERR_INVALID_ARG
-    assert lib.chorus_mask_from_mass(None, 4, 64, C.c_float(0.9), C.c_float(0.1), fake, None, None) == B.CHORUS_ERR_INVALID_ARG
+    assert lib.chorus_mask_from_mass(fake, 4, 4096, C.c_double(0.9), C.c_double(0.1), fake, None, None) == B.CHORUS_ERR_UNSUPPORTED
+    assert lib.chorus_mask_from_mass(fake, 4, 64, C.c_double(1.5), C.c_double(0.1), fake, None, None) == B.CHORUS_ERR_INVALID_ARG
+    assert lib.chorus_mask_from_mass(fake, 0, 64, C.c_double(0.9), C.c_double(0.1), fake, None, None) == B.CHORUS_ERR_INVALID_ARG
+    assert lib.chorus_mask_from_mass(None, 4, 64, C.c_double(0.9), C.c_double(0.1), fake, None, None) == B.CHORUS_ERR_INVALID_ARG
     assert lib.chorus_mask_coverage(fake, fake, 0, 1, 1, fake, None) == B.CHORUS_ERR_INVALID_ARG
     assert lib.chorus_head_costs(None, 4, 4, fake, None) == B.CHORUS_ERR_INVALID_ARG
     assert lib.chorus_schedule_heads(None, 4, 2, fake, None) == B.CHORUS_ERR_INVALID_ARG
@@ -84,6 +84,12 @@ def test_argument_validation_on_host(lib):
                                               fake, C.byref(shp64), None, fake, None)
     assert st == B.CHORUS_ERR_UNSUPPORTED          # FP16 is a known dtype; d = 64 is what is refused
     assert b"head_dim" in lib.chorus_last_error()
+    # scale must be positive and finite (the row maximum is taken on the raw scores)
+    for bad in (0.0, -0.088, float("nan"), float("inf")):
+        st = lib.chorus_block_sparse_attn_fwd(fake, fake, fake, fake, fake, C.c_float(bad), B.CHORUS_BF16,
+                                              fake, C.byref(shp), None, None)
+        assert st == B.CHORUS_ERR_INVALID_ARG and b"scale" in lib.chorus_last_error(), bad
+        assert lib.chorus_block_mass(fake, fake, C.c_float(bad), C.byref(shp), None, fake, None) == B.CHORUS_ERR_INVALID_ARG
 
 
 def test_product_path_does_not_touch_the_oracle():

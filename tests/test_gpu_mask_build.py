@@ -13,7 +13,6 @@ from paper_2606_25040_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-F = lambda x: float(np.float32(x))      # the ABI takes float: the oracle gets the same value
 
 
 def mass_close(got, ref):
@@ -58,7 +57,9 @@ def test_block_mass_is_deterministic():
     assert torch.equal(a, b)
 
 
-@pytest.mark.parametrize("nk", [1, 31, 32, 33, 64, 257, 512, 1182, 2048])
+# nk = 70, 590, 640: min_top_k * nk = 0.1 * nk is an exact integer there (R22: the floor is
+# ceil of the DOUBLE product, 0.1 x 70 = 7 blocks, not 8 as a float32 0.1 would give)
+@pytest.mark.parametrize("nk", [1, 31, 32, 33, 64, 70, 257, 512, 590, 640, 1182, 2048])
 def test_mask_from_mass_bit_exact(nk):
     g = np.random.default_rng(nk)
     rows = 37
@@ -67,12 +68,14 @@ def test_mask_from_mass_bit_exact(nk):
     mass[2, : (nk + 1) // 2] = mass[2, 0]            # ties
     mass[3] = np.float32(1.0)                        # all equal: index order decides
     dm = torch.from_numpy(mass).to(dev())
-    for top_p, k_min in ((0.95, 0.1), (0.9, 0.0), (0.5, 0.3), (1.0, 0.0), (0.0, 0.0), (0.0, 1.0)):
-        bm_o, kept_o = oracle.mask_from_mass(mass, nk, F(top_p), F(k_min))
+    for top_p, k_min in ((0.95, 0.1), (0.9, 0.0), (0.5, 0.3), (1.0, 0.0), (0.0, 0.0), (0.0, 1.0), (0.0, 0.1)):
+        bm_o, kept_o = oracle.mask_from_mass(mass, nk, top_p, k_min)
         bm, kept = B.chorus_mask_from_mass(dm, top_p, k_min)
         torch.cuda.synchronize()
         assert np.array_equal(bm.cpu().numpy().view(np.uint32), bm_o), (nk, top_p, k_min)
         assert np.array_equal(kept.cpu().numpy(), kept_o)
+        if top_p == 0.0 and k_min == 0.1 and nk in (70, 590, 640):
+            assert int(kept_o.max()) == nk // 10
 
 
 def test_mask_coverage_matches_oracle():
@@ -106,14 +109,14 @@ def test_true_top_p_mask_of_one_full_size_head():
         mass_close(m[0, 0, qb].astype(np.float64), ref[0, 0, qb])
     top_p, k_min = 0.9, 0.1
     bm, kept = B.chorus_mask_from_mass(mass[0], top_p, k_min)
-    bm_o, kept_o = oracle.mask_from_mass(m[0], cfg.nk, F(top_p), F(k_min))
+    bm_o, kept_o = oracle.mask_from_mass(m[0], cfg.nk, top_p, k_min)
     torch.cuda.synchronize()
     assert np.array_equal(bm.cpu().numpy().view(np.uint32), bm_o)
     cov = B.chorus_mask_coverage(mass[0], bm, cfg.nk).cpu().numpy()
     assert np.allclose(cov, oracle.mask_coverage(m[0], bm_o, cfg.nk), atol=2e-6)
     assert (cov >= 0.9 - 1e-5).all()
     k = kept.cpu().numpy()
-    assert k.min() >= int(np.ceil(F(k_min) * cfg.nk)) and k.max() <= cfg.nk
+    assert k.min() >= int(np.ceil(k_min * cfg.nk)) and k.max() <= cfg.nk
     # the mask feeds the reuse path unchanged
     rp, ci = B.chorus_mask_to_index(bm[None], cfg.nk)
     rp_o, ci_o = oracle.mask_to_index(bm_o[None], cfg.nk)
@@ -189,7 +192,7 @@ def test_cross_request_mask_reuse_end_to_end():
     src_mask, kept = B.chorus_mask_from_mass(src_mass[0], 0.9, 0.1)            # the cached artefact
     torch.cuda.synchronize()
     assert kept.float().mean().item() / nk < 0.5
-    src_mask_o, _ = oracle.mask_from_mass(oracle.block_mass(Qs, Ks, scale)[0].astype(np.float32), nk, F(0.9), F(0.1))
+    src_mask_o, _ = oracle.mask_from_mass(oracle.block_mass(Qs, Ks, scale)[0].astype(np.float32), nk, 0.9, 0.1)
     agree = (W.unpack_bits(src_mask.cpu().numpy().view(np.uint32), nk) == W.unpack_bits(src_mask_o, nk)).mean()
     assert agree > 0.995            # masses differ in the last bits, so a few threshold blocks may differ
 
