@@ -354,6 +354,10 @@ const char* chorus_version(void);
 int64_t chorus_launch_count(void);
 void chorus_reset_launch_count(void);
 
+/* TMA tensor maps are cached per thread, keyed by (pointer, element size, shape, strides, box): a call with
+ * tensors seen before encodes nothing.  Number of cuTensorMapEncodeTiled calls made on this thread so far. */
+int64_t chorus_tensor_map_encodes(void);
+
 #ifdef __cplusplus
 }
 #endif

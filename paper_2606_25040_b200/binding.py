@@ -23,7 +23,7 @@ EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_
            "chorus_mask_to_index_64x128", "chorus_block_sparse_attn_fwd_64x128", "chorus_block_mass_64x128",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
            "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_gather_heads", "chorus_scatter_heads", "chorus_last_error", "chorus_version",
-           "chorus_launch_count", "chorus_reset_launch_count"]
+           "chorus_launch_count", "chorus_reset_launch_count", "chorus_tensor_map_encodes"]
 
 
 class ChorusError(RuntimeError):
@@ -55,6 +55,7 @@ def lib() -> C.CDLL:
         L.chorus_last_error.restype = C.c_char_p
         L.chorus_version.restype = C.c_char_p
         L.chorus_launch_count.restype = C.c_int64
+        L.chorus_tensor_map_encodes.restype = C.c_int64
         L.chorus_mask_to_index.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p,
                                            C.c_void_p, C.c_int64, C.c_void_p,
                                            C.POINTER(C.c_size_t), C.c_void_p]
@@ -113,6 +114,10 @@ def chorus_version() -> str:
 
 def chorus_launch_count() -> int:
     return int(lib().chorus_launch_count())
+
+
+def chorus_tensor_map_encodes() -> int:
+    return int(lib().chorus_tensor_map_encodes())
 
 
 def chorus_reset_launch_count() -> None:

@@ -31,20 +31,61 @@ EncodeTiledFn get_encode_fn() {
 
 // Tensor map over a [B][N][H][d]-indexed tensor with element strides (d contiguous):
 // dims (innermost first) = {d, N, H, B}; box = {box_cols, box_rows, 1, 1}; 128-byte swizzle.
+// Encoded maps are kept in a small per-thread cache keyed by everything that goes into the encoding
+// (SURVEY section 8(b)): a serving loop calls with the same few tensors over and over, and
+// cuTensorMapEncodeTiled costs a few microseconds of host time per map.
+struct TmapKey {
+    const void* base;
+    int elem_bytes, B, H, N, d, box_cols, box_rows;
+    int64_t sb, sn, sh;
+    bool operator==(const TmapKey& o) const {
+        return base == o.base && elem_bytes == o.elem_bytes && B == o.B && H == o.H && N == o.N && d == o.d &&
+               box_cols == o.box_cols && box_rows == o.box_rows && sb == o.sb && sn == o.sn && sh == o.sh;
+    }
+};
+constexpr int TMAP_CACHE = 1024, TMAP_PROBES = 8;     // hashed, 8-way probing, the first probe is the victim
+struct TmapCache {
+    TmapKey key[TMAP_CACHE];
+    CUtensorMap map[TMAP_CACHE];
+    bool used[TMAP_CACHE];
+};
+thread_local TmapCache* g_tmaps = nullptr;
+thread_local int64_t g_tmap_encodes = 0;
+
+uint32_t tmap_hash(const TmapKey& k) {
+    uint64_t h = reinterpret_cast<uintptr_t>(k.base) * 0x9E3779B97F4A7C15ull;
+    h ^= (static_cast<uint64_t>(k.box_rows) << 40) ^ (static_cast<uint64_t>(k.elem_bytes) << 32) ^ static_cast<uint64_t>(k.sn) ^
+         (static_cast<uint64_t>(k.N) << 13);
+    h *= 0xC2B2AE3D27D4EB4Full;
+    return static_cast<uint32_t>(h >> 40);
+}
+
 chorus_status make_tmap(CUtensorMap* tm, const void* base, int elem_bytes, int B, int H, int N,
                         int d, int64_t sb, int64_t sn, int64_t sh, int box_cols, int box_rows,
                         const char* name) {
+    // a size-1 dimension never advances; give it a harmless, valid stride
+    const int64_t row = static_cast<int64_t>(d);
+    if (N == 1) sn = row;
+    if (H == 1) sh = row;
+    if (B == 1) sb = row;
+    const TmapKey k{base, elem_bytes, B, H, N, d, box_cols, box_rows, sb, sn, sh};
+    if (!g_tmaps) g_tmaps = new TmapCache();          // zero-initialised: nothing used
+    const uint32_t h0 = tmap_hash(k);
+    int slot = static_cast<int>(h0 % TMAP_CACHE);
+    for (int i = 0; i < TMAP_PROBES; ++i) {
+        const int s = static_cast<int>((h0 + i) % TMAP_CACHE);
+        if (!g_tmaps->used[s]) { slot = s; break; }
+        if (g_tmaps->key[s] == k) {
+            *tm = g_tmaps->map[s];
+            return CHORUS_OK;
+        }
+    }
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return set_error(CHORUS_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
     const CUtensorMapDataType dt =
         elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8;
     cuuint64_t dims[4] = {static_cast<cuuint64_t>(d), static_cast<cuuint64_t>(N),
                           static_cast<cuuint64_t>(H), static_cast<cuuint64_t>(B)};
-    // a size-1 dimension never advances; give it a harmless, valid stride
-    const int64_t row = static_cast<int64_t>(d);
-    if (N == 1) sn = row;
-    if (H == 1) sh = row;
-    if (B == 1) sb = row;
     cuuint64_t strides[3] = {static_cast<cuuint64_t>(sn) * elem_bytes,
                              static_cast<cuuint64_t>(sh) * elem_bytes,
                              static_cast<cuuint64_t>(sb) * elem_bytes};
@@ -56,6 +97,10 @@ chorus_status make_tmap(CUtensorMap* tm, const void* base, int elem_bytes, int B
     if (r != CUDA_SUCCESS)
         return set_error(CHORUS_ERR_CUDA, "cuTensorMapEncodeTiled(%s) failed with CUresult %d", name,
                          static_cast<int>(r));
+    ++g_tmap_encodes;
+    g_tmaps->key[slot] = k;
+    g_tmaps->map[slot] = *tm;
+    g_tmaps->used[slot] = true;
     return CHORUS_OK;
 }
 
@@ -91,6 +136,7 @@ const char* chorus_version(void) {
 }
 
 int64_t chorus_launch_count(void) { return g_launches; }
+int64_t chorus_tensor_map_encodes(void) { return g_tmap_encodes; }
 void chorus_reset_launch_count(void) { g_launches = 0; }
 
 chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,

@@ -61,6 +61,30 @@ def sample_items(H, nq, n, seed, always=()):
     return sorted(picks)
 
 
+def stratified_items(H, nq, per_head, seed):
+    """per_head (head, query-block) items in EVERY head: the first and the last (ragged) query block always,
+    the rest drawn without replacement."""
+    g = np.random.default_rng(seed)
+    out = []
+    for h in range(H):
+        mid = g.choice(np.arange(1, nq - 1), size=min(per_head - 2, max(nq - 2, 0)), replace=False) if nq > 2 else []
+        out += [(0, h, 0)] + [(0, h, int(q)) for q in sorted(mid)] + ([(0, h, nq - 1)] if nq > 1 else [])
+    return out
+
+
+def report(name, **kv):
+    """Append measured parity figures to gpurun_out/parity_report.jsonl (scratch; the figures that matter are
+    quoted in DESIGN.md section 5) and print them."""
+    import json
+    import os
+    d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    os.makedirs(d, exist_ok=True)
+    line = json.dumps({"test": name, **kv})
+    print(line)
+    with open(os.path.join(d, "parity_report.jsonl"), "a") as f:
+        f.write(line + "\n")
+
+
 def err_stats(got, ref):
     e = np.abs(got - ref)
     relfro = np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-30)

@@ -8,8 +8,8 @@ import pytest
 import torch
 
 import oracle
-from gpu_common import (FP8_COS, FP8_MAX, all_items, dbf16, dmask, err_stats, gather_items,
-                        sample_items)
+from gpu_common import (FP8_COS, FP8_MAX, all_items, dbf16, dmask, err_stats, gather_items, report,
+                        sample_items, stratified_items)
 from paper_2606_25040_b200 import binding as B
 from paper_2606_25040_b200 import workloads as W
 
@@ -69,7 +69,14 @@ def compare(cfg, Q, K, V, bm, items, stress=False):
         # two bf16 output roundings.
         bound = e4m3_weight_bound(q8, k8, v8, qs, ks, vs, bm, cfg, items)
         tol = np.maximum(FP8_MAX, 1.1 * bound + 1e-3) + 2.0 ** -8 * np.abs(ref)
-        assert np.all(np.abs(got - ref) <= tol), (mx, float((np.abs(got - ref) - tol).max()))
+        err = np.abs(got - ref)
+        assert np.all(err <= tol), (mx, float((err - tol).max()))
+        # distance from the PLAIN north_star bound (8e-2 on N(0,1) inputs): reported, DESIGN.md section 5
+        over = err > FP8_MAX
+        report("fp8_stress_" + cfg.name, items=len(items), elements=int(err.size), over_plain_bound=int(over.sum()),
+               max_abs=mx, cos=cos, relfro=relfro,
+               min_abs_ref_where_over=float(np.abs(ref[over]).min()) if over.any() else None,
+               max_err_over_first_order_bound=float((err[over] / bound[over]).max()) if over.any() else None)
     else:
         assert mx <= FP8_MAX, mx
     assert cos >= FP8_COS and relfro <= FP8_RELFRO, (cos, relfro)
@@ -131,7 +138,7 @@ def test_cfg3_480p_sampled_blocks_full_size():
     cfg = W.CFG2
     Q, K, V = W.qkv_bits(cfg)
     bm = W.layer_mask(cfg)
-    items = sample_items(cfg.H, cfg.nq, 10, seed=0, always=[(0, 0, 0), (0, cfg.H - 1, cfg.nq - 1)])
+    items = stratified_items(cfg.H, cfg.nq, 8, seed=0)       # all 40 heads x 8 query blocks: 320 items
     O8, stats = compare(cfg, Q, K, V, bm, items)
     # reported, not gated: total quantisation cost against the BF16 path on the unquantised inputs
     rp, ci = B.chorus_mask_to_index(dmask(bm[None]), cfg.nk)
@@ -148,7 +155,7 @@ def test_cfg4_720p_stress_rows_sampled_blocks():
     cfg = W.scaled(W.CFG4, H=4)
     Q, K, V = W.qkv_bits(cfg)
     bm = W.layer_mask(cfg)
-    items = sample_items(cfg.H, cfg.nq, 5, seed=1, always=[(0, 3, cfg.nq - 1)])
+    items = stratified_items(cfg.H, cfg.nq, 6, seed=1)
     compare(cfg, Q, K, V, bm, items, stress=True)
 
 

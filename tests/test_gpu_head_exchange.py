@@ -67,7 +67,7 @@ def test_scheduled_round_trip_around_the_attention_kernel_one_rank():
     order = order.reshape(-1).tolist()
     assert sorted(order) == list(range(cfg.H)) and order != list(range(cfg.H))
     # one rank: the "exchange" is the head permutation alone
-    qh, kh, vh = (ulysses.seq_to_heads(x, order) for x in (q, k, v))
+    qh, kh, vh = (ulysses.seq_to_heads(x, order, cfg.N) for x in (q, k, v))
     assert np.array_equal(qh[0].cpu().view(torch.int16).numpy().view(np.uint16), Q[0][:, order])
     rp2, ci2 = B.chorus_mask_to_index(dmask(bm[order][None]), cfg.nk)      # the masks follow their heads
     oh = B.chorus_block_sparse_attn_fwd(qh, kh, vh, rp2, ci2, cfg.scale)

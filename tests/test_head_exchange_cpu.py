@@ -1,6 +1,7 @@
 """CPU tests of the head exchange (appendix A): pins of the oracle's gather / scatter copies, and the
-data flow of paper_2606_25040_b200.ulysses over a 2-rank gloo group with the oracle's copies in place of the CUDA
-kernels (the exchange logic, chunk order and views are the product's; no GPU here)."""
+exchange functions of paper_2606_25040_b200.ulysses over a 2-rank gloo group, composed here with the oracle's copies
+(the all-to-all, its split sizes for unequal shards and the views are the product's; the CUDA copies around them are
+tested on the GPU in test_gpu_head_exchange.py and, with two ranks over NCCL, in test_gpu_ulysses_nccl.py)."""
 import os
 import socket
 
@@ -36,28 +37,32 @@ def _worker(rank, world, port, q):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         from paper_2606_25040_b200 import ulysses
-        N, H, d = 12, 6, 4
-        g = np.random.default_rng(0)
-        X = g.standard_normal((N, H, d)).astype(np.float32)                     # the global tensor
-        order = [4, 1, 3, 0, 5, 2]                                              # rank 0: 4, 1, 3; rank 1: 0, 5, 2
-        n_loc, slots = N // world, H // world
-        x_loc = torch.from_numpy(X[rank * n_loc:(rank + 1) * n_loc].copy())[None]
-        gather = lambda x, o, P: torch.from_numpy(oracle.gather_heads(x.numpy(), o, P))
-
-        def scatter(chunks, o, out):
-            out.copy_(torch.from_numpy(oracle.scatter_heads(chunks.numpy(), o)))
-
-        xh = ulysses.seq_to_heads(x_loc, order, _gather=gather)
-        mine = order[rank * slots:(rank + 1) * slots]
-        ok1 = xh.shape == (1, N, slots, d) and np.array_equal(xh[0].numpy(), X[:, mine])   # all tokens, my heads
-        # "attention" = something per (token, head) that depends on the global token index
-        oh = xh * 2.0 + torch.arange(N, dtype=torch.float32)[None, :, None, None]
-        back = ulysses.heads_to_seq(oh.contiguous(), order, _scatter=scatter)
-        ref = (X * 2.0 + np.arange(N, dtype=np.float32)[:, None, None])[rank * n_loc:(rank + 1) * n_loc]
-        ok2 = back.shape == (1, n_loc, H, d) and np.array_equal(back[0].numpy(), ref)
+        oks = []
+        for N in (12, 13):                                                          # equal and unequal shards
+            H, d = 6, 4
+            g = np.random.default_rng(0)
+            X = g.standard_normal((N, H, d)).astype(np.float32)                     # the global tensor
+            order = [4, 1, 3, 0, 5, 2]                                              # rank 0: 4, 1, 3; rank 1: 0, 5, 2
+            bounds = ulysses.shard_bounds(N, world)
+            lo, hi = bounds[rank], bounds[rank + 1]
+            slots = H // world
+            # the local copies are the oracle's here (no GPU); the exchange, split sizes and views are the product's
+            packed = torch.from_numpy(oracle.gather_heads(X[lo:hi].copy(), order, world))
+            xh = ulysses.exchange_to_heads(packed, bounds)
+            mine = order[rank * slots:(rank + 1) * slots]
+            oks.append(tuple(xh.shape) == (N, slots, d) and np.array_equal(xh.numpy(), X[:, mine]))   # all tokens, my heads
+            # "attention" = something per (token, head) that depends on the global token index
+            oh = xh * 2.0 + torch.arange(N, dtype=torch.float32)[:, None, None]
+            chunks = ulysses.exchange_to_seq(oh.contiguous(), bounds)
+            back = oracle.scatter_heads(chunks.numpy(), order)
+            ref = (X * 2.0 + np.arange(N, dtype=np.float32)[:, None, None])[lo:hi]
+            oks.append(back.shape == (hi - lo, H, d) and np.array_equal(back, ref))
         rows = ulysses.rank_rows(order, rank, world, nq_blk=5)
-        ok3 = rows == [(h, 5 * h, 5 * h + 5) for h in mine]
-        q.put((rank, bool(ok1), bool(ok2), bool(ok3)))
+        oks.append(rows == [(h, 5 * h, 5 * h + 5) for h in mine])
+        oks.append(ulysses.shard_bounds(13, 2) == [0, 6, 13] and ulysses.shard_bounds(32760, 8)[1] == 4095)
+        oks.append(abs(ulysses.imbalance([4, 1, 1, 1, 1, 4], [0, 1, 2, 3, 4, 5], 2) - 1.0) < 1e-12 and
+                   abs(ulysses.imbalance([4, 4, 1, 1, 1, 1], [0, 1, 2, 3, 4, 5], 2) - 9 / 6) < 1e-12)
+        q.put((rank, all(bool(o) for o in oks), len(oks)))
     finally:
         dist.destroy_process_group()
 
@@ -73,4 +78,4 @@ def test_ulysses_data_flow_two_ranks_gloo():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    assert res == [(0, True, True, True), (1, True, True, True)]
+    assert res == [(0, True, 7), (1, True, 7)]

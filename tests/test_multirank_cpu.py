@@ -42,6 +42,21 @@ def test_single_rank_is_identity_and_aggregate_scales_with_replicas():
     assert bench.whole_job_value(8, 5.5e12, 4.4) == 8 * one      # weak scaling: same time, 8x the work
 
 
+def test_ulysses_plan_is_deterministic_and_balances():
+    # bench.py --mode ulysses: every rank derives the same head order from the same costs (no exchange needed),
+    # and the greedy schedule never makes the max / mean load worse than the index order
+    import numpy as np
+    cost = [int(c) for c in np.random.default_rng(77).uniform(0.10, 0.40, 40) * 131072]
+    for ranks in (1, 2, 4, 8):
+        order, plan = bench.ulysses_plan(cost, ranks)
+        assert sorted(order) == list(range(40))
+        assert bench.ulysses_plan(cost, ranks)[0] == order
+        assert plan["imbalance_max_over_avg_after"] <= plan["imbalance_max_over_avg_before"] + 1e-12
+        assert plan["imbalance_max_over_avg_after"] >= 1.0 - 1e-12
+    assert bench.ulysses_plan(cost, 1)[0] == list(range(40))          # one rank: a no-op (Table 4)
+    assert bench.ulysses_plan(cost, 8)[1]["imbalance_max_over_avg_after"] < 1.06
+
+
 def test_reference_arm_prints_the_contract_line():
     # bench.py --impl reference: the oracle on the host cores, one JSON line with the base contract's keys
     import json
