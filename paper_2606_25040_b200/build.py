@@ -14,8 +14,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libchorus.so")
-SOURCES = ["chorus_api.cu", "mask_decode.cu", "retrieve.cu", "quantize_fp8.cu", "attn_fwd.cu", "mask_build.cu", "head_schedule.cu", "head_exchange.cu"]
-HEADERS = ["chorus_internal.h", "sm100_ptx.cuh", os.path.join("..", "..", "include", "chorus.h")]
+SOURCES = ["chorus_api.cu", "mask_decode.cu", "retrieve.cu", "quantize_fp8.cu", "attn_fwd.cu", "attn_fwd_fp8.cu", "mask_build.cu", "head_schedule.cu", "head_exchange.cu"]
+HEADERS = ["chorus_internal.h", "sm100_ptx.cuh", "attn_common.cuh", os.path.join("..", "..", "include", "chorus.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
          "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall"]

@@ -32,18 +32,15 @@
 // 64-key tile and V's per-channel scale applied in the epilogue.
 #include <cuda_bf16.h>
 
-#include "chorus_internal.h"
-#include "sm100_ptx.cuh"
+#include "attn_common.cuh"
 
 namespace chorus {
 namespace {
 
 using namespace ptx;
+using namespace attn;
 
-constexpr int BQ = 128, BK = 64;
 constexpr int SBUFS = 3;
-constexpr int NUM_THREADS = 384;
-constexpr int PRODUCER_WARP = 8, MMA_WARP = 9;
 
 // Per-dtype geometry.  A "slab" is a [128 rows][128 B] swizzled tile: 64 bf16 channels or all 128
 // e4m3 channels of 128 rows (one Q block, or the two 64-key tiles of a pair).
@@ -87,55 +84,6 @@ constexpr uint32_t TM_S = 0, TM_O = 384, TM_COLS = 512;
 // named barriers: 0 = __syncthreads, 1..4 = warp pair (w, w+4) in the epilogue, 5..6 = column-half
 // warpgroup, 7..14 = m_ref hand-off published by parity 0 (7..10) / parity 1 (11..14) of quarter wq
 constexpr uint32_t NB_PAIR = 1, NB_HALF = 5, NB_HAND = 7;
-
-__device__ __forceinline__ void setmaxnreg_inc_216() { asm volatile("setmaxnreg.inc.sync.aligned.u32 216;"); }
-__device__ __forceinline__ void setmaxnreg_dec_56() { asm volatile("setmaxnreg.dec.sync.aligned.u32 56;"); }
-
-template <bool V>
-struct BoolTag {
-    static constexpr bool value = V;
-};
-
-struct Item {
-    int b, h, qb, r0, nt, np;
-};
-__device__ __forceinline__ Item get_item(const AttnParams& p, int idx) {
-    Item it;
-    it.qb = idx % p.nq;
-    const int bh = idx / p.nq;
-    it.h = bh % p.H;
-    it.b = bh / p.H;
-    const int row = it.h * p.nq + it.qb;
-    it.r0 = __ldg(p.row_ptr + row);
-    it.nt = __ldg(p.row_ptr + row + 1) - it.r0;
-    it.np = (it.nt + 1) >> 1;
-    return it;
-}
-
-// the same, with every field broadcast from lane 0: the compiler then knows the values are
-// warp-uniform (needed by the converged producer / MMA warps)
-__device__ __forceinline__ Item get_item_uniform(const AttnParams& p, int idx) {
-    Item it = get_item(p, idx);
-    it.r0 = __shfl_sync(0xffffffffu, it.r0, 0);
-    it.nt = __shfl_sync(0xffffffffu, it.nt, 0);
-    it.np = (it.nt + 1) >> 1;
-    return it;
-}
-
-__device__ __forceinline__ float max3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
-
-// max of 64 fp32 bit patterns
-__device__ __forceinline__ float max64(const uint32_t* sv) {
-    float a0 = -INFINITY, a1 = -INFINITY, a2 = -INFINITY, a3 = -INFINITY;
-#pragma unroll
-    for (int k = 0; k < 64; k += 8) {
-        a0 = max3(a0, __uint_as_float(sv[k]), __uint_as_float(sv[k + 1]));
-        a1 = max3(a1, __uint_as_float(sv[k + 2]), __uint_as_float(sv[k + 3]));
-        a2 = max3(a2, __uint_as_float(sv[k + 4]), __uint_as_float(sv[k + 5]));
-        a3 = max3(a3, __uint_as_float(sv[k + 6]), __uint_as_float(sv[k + 7]));
-    }
-    return fmaxf(fmaxf(a0, a1), fmaxf(a2, a3));
-}
 
 // kBeta: first-frame key enhancement (eq. (1)) as a factor on the scores of keys < n_first
 // kHalf: col_idx entries carry per-half flags (bit 30 / 31: query rows 0-63 / 64-127 of the block do NOT keep the
@@ -251,7 +199,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             constexpr uint32_t FMT = (kFp8 || kF16) ? 0u : 1u;   // kind::f16: 0 = fp16, 1 = bf16
             constexpr uint32_t IDESC_S128 = make_idesc(FMT, FMT, 128, 128, 0, 0);
             constexpr uint32_t IDESC_S64 = make_idesc(FMT, FMT, 128, 64, 0, 0);
-            constexpr uint32_t IDESC_PV = make_idesc(FMT, FMT, 128, 128, 0, 1);
+            constexpr uint32_t IDESC_PV = make_idesc(FMT, FMT, 128, 128, 0, 1);   // A and B formats must agree in kind::f16
             const uint64_t dQ = smem_desc_sw128(sQ, 16, 1024);
             const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
             const uint64_t dV = smem_desc_sw128(sV, 16384, 1024);
@@ -704,7 +652,7 @@ cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, cons
         return launch_one<F8, F16, false, false>(tmQ, tmK, tmV, tmO, p, stream);
     };
     if (dtype == CHORUS_BF16) return go(BoolTag<false>{}, BoolTag<false>{});
-    if (dtype == CHORUS_FP8_E4M3) return go(BoolTag<true>{}, BoolTag<false>{});
+    if (dtype == CHORUS_FP8_E4M3) return launch_attn_fwd_fp8(tmQ, tmK, tmV, tmO, p, stream);
     if (dtype == CHORUS_FP16) return go(BoolTag<false>{}, BoolTag<true>{});
     return cudaErrorNotSupported;
 }

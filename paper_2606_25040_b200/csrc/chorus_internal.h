@@ -56,6 +56,10 @@ cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, cons
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
                             cudaStream_t stream);
 
+// attn_fwd_fp8.cu: the e4m3 kernel (launch_attn_fwd dispatches to it)
+cudaError_t launch_attn_fwd_fp8(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
+                                const CUtensorMap& tmO, const AttnParams& p, cudaStream_t stream);
+
 // ---- mask_build.cu -----------------------------------------------------------------------------
 cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, const float* lse, float* mass,
                               int B, int H, int N, float scale_log2, bool geo64, cudaStream_t stream);

@@ -14,6 +14,24 @@ from paper_2606_25040_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 
+def weighted_abs_v(Q, K, V, bm, cfg, items, scale):
+    """A[i, c] = sum_j w_ij |v_jc| over the retained keys, in numpy fp64 straight from the definition (independent of
+    the oracle and of the kernel).  The kernel feeds bf16-rounded weights to P V and divides by the fp32 sum of the
+    unrounded ones, so a weight's rounding (relative 2^-9) reaches the output as 2^-9 w_ij |v_jc|: averaged away over
+    thousands of comparable keys, but not on a row that a single key dominates (cfg4's x8 rows), where A ~ |O|."""
+    keep = W.unpack_bits(bm, cfg.nk)
+    f = lambda b: W.f32_from_bf16_bits(b).astype(np.float64)
+    out = np.zeros((len(items), 128, 128))
+    for t, (b, h, qb) in enumerate(items):
+        lo, hi = qb * 128, min(cfg.N, qb * 128 + 128)
+        idx = np.concatenate([np.arange(kb * 64, min(cfg.N, kb * 64 + 64)) for kb in np.nonzero(keep[h, qb])[0]])
+        sc = scale * (f(Q[b, lo:hi, h]) @ f(K[b, idx, h]).T)
+        w = np.exp(sc - sc.max(axis=1, keepdims=True))
+        w /= w.sum(axis=1, keepdims=True)
+        out[t, : hi - lo] = w @ np.abs(f(V[b, idx, h]))
+    return out
+
+
 def compare(cfg, Q, K, V, bm, items, scale=None, tight=True, stress=False):
     scale = cfg.scale if scale is None else scale
     O = gpu_attention(Q, K, V, bm, cfg.nk, scale)
@@ -22,18 +40,23 @@ def compare(cfg, Q, K, V, bm, items, scale=None, tight=True, stress=False):
     got = gather_items(O, items, cfg.N)
     mx, mean, relfro, cos = err_stats(got, ref)
     if stress:
-        # x8 rows give outputs of magnitude ~25, where the bf16 OUTPUT format alone rounds by
-        # 2^-9 |O| ~ 0.05: the absolute 2e-2 bound is stated for N(0,1) inputs (north_star), so it
-        # is applied to the error in excess of two bf16 roundings
+        # x8 rows give outputs of magnitude ~25, where the bf16 OUTPUT format alone rounds by up to
+        # 2^-8 |O| ~ 0.1, and a row dominated by one key carries the bf16 rounding of that one weight
+        # un-averaged (2^-9 A, A = sum_j w_ij |v_jc| ~ |O| there).  north_star's absolute 2e-2 is stated
+        # for N(0,1) inputs, so it is applied to the error in excess of these two roundings, both
+        # computed here from the definitions.
         err = np.abs(got - ref)
-        assert np.all(err <= BF16_MAX + 2.0 ** -8 * np.abs(ref)), mx
+        A = weighted_abs_v(Q, K, V, bm, cfg, items, scale)
+        tol = BF16_MAX + 2.0 ** -8 * np.abs(ref) + 2.0 ** -9 * A
+        assert np.all(err <= tol), (mx, float((err - tol).max()))
         assert mean <= BF16_MEAN and relfro <= BF16_RELFRO, (mean, relfro)
         # how far this is from the PLAIN north_star bound: count and size of the elements beyond 2e-2, and
-        # every one of them must sit where one bf16 output rounding (2^-9 |ref|) alone exceeds 1e-2
+        # every one of them must sit where one bf16 output rounding (up to 2^-8 |ref|) alone exceeds 1e-2
         over = err > BF16_MAX
-        assert np.all(2.0 ** -9 * np.abs(ref[over]) > 1e-2), float(np.abs(ref[over]).min())
+        assert np.all(2.0 ** -8 * np.abs(ref[over]) > 1e-2), float(np.abs(ref[over]).min())
         report("bf16_stress_" + cfg.name, items=len(items), elements=int(err.size), over_plain_bound=int(over.sum()),
-               max_abs=mx, mean_abs=mean, relfro=relfro,
+               max_abs=mx, mean_abs=mean, relfro=relfro, max_err_over_tol=float((err / tol).max()),
+               over_output_rounding_alone=int((err > BF16_MAX + 2.0 ** -8 * np.abs(ref)).sum()),
                min_abs_ref_where_over=float(np.abs(ref[over]).min()) if over.any() else None,
                max_err_over_bf16_ulp_of_ref=float((err[over] / (2.0 ** -8 * np.abs(ref[over]))).max()) if over.any() else None)
         return O
