@@ -26,6 +26,8 @@ def lib():
         _lib = C.CDLL(_build())
         _lib.oracle_mask_to_index.restype = C.c_int64
         _lib.oracle_mask_to_index_64x128.restype = C.c_int64
+        _lib.oracle_mask_to_index_u16.restype = C.c_int64
+        _lib.oracle_mask_to_index_64x128_u16.restype = C.c_int64
         _lib.oracle_e4m3_to_double.restype = C.c_double
         _lib.oracle_e4m3_to_double.argtypes = [C.c_uint8]
         _lib.oracle_f16_to_double.restype = C.c_double
@@ -74,6 +76,34 @@ def mask_to_index_64x128(bitmask: np.ndarray, N: int):
     nnz = lib().oracle_mask_to_index_64x128(_p(bm), L, H, N, _p(row_ptr), None)
     col_idx = np.zeros(max(int(nnz), 1), dtype=np.uint32)
     lib().oracle_mask_to_index_64x128(_p(bm), L, H, N, _p(row_ptr), _p(col_idx))
+    return row_ptr, col_idx[:nnz]
+
+
+def mask_to_index_u16(bitmask: np.ndarray, nk: int):
+    """mask_to_index with 16-bit entries (nk <= 65536): (row_ptr int32, col_idx uint16)."""
+    bm = _c(bitmask, np.uint32)
+    L, H, nq, words = bm.shape
+    assert words == (nk + 31) // 32
+    row_ptr = np.zeros(L * H * nq + 1, dtype=np.int32)
+    nnz = lib().oracle_mask_to_index_u16(_p(bm), L, H, nq, nk, _p(row_ptr), None)
+    if nnz < 0:
+        raise ValueError("key-block index does not fit 16 bits")
+    col_idx = np.zeros(max(int(nnz), 1), dtype=np.uint16)
+    lib().oracle_mask_to_index_u16(_p(bm), L, H, nq, nk, _p(row_ptr), _p(col_idx))
+    return row_ptr, col_idx[:nnz]
+
+
+def mask_to_index_64x128_u16(bitmask: np.ndarray, N: int):
+    """mask_to_index_64x128 with 16-bit entries: tile | bit 14 = upper half does not keep it | bit 15 = lower."""
+    bm = _c(bitmask, np.uint32)
+    L, H, nq64, words = bm.shape
+    assert nq64 == (N + 63) // 64 and words == ((N + 127) // 128 + 31) // 32
+    row_ptr = np.zeros(L * H * ((N + 127) // 128) + 1, dtype=np.int32)
+    nnz = lib().oracle_mask_to_index_64x128_u16(_p(bm), L, H, N, _p(row_ptr), None)
+    if nnz < 0:
+        raise ValueError("tile index does not fit 14 bits")
+    col_idx = np.zeros(max(int(nnz), 1), dtype=np.uint16)
+    lib().oracle_mask_to_index_64x128_u16(_p(bm), L, H, N, _p(row_ptr), _p(col_idx))
     return row_ptr, col_idx[:nnz]
 
 

@@ -19,6 +19,9 @@
 //                               keys, closed form; 64 x 128 geometry: numpy token-level masked softmax
 //   oracle_mask_to_index_64x128 pinned (brute-force restatement, round trip to the token-level keep
 //                               matrix of the mask, ascending / no duplicates)
+//   oracle_mask_to_index_u16, oracle_mask_to_index_64x128_u16
+//                               pinned (independent per-bit Python loops, agreement with the 32-bit forms
+//                               entry by entry, flag positions, the does-not-fit refusals)
 //   oracle_quantize_fp8         pinned (torch.float8_e4m3fn cast as an independent library routine,
 //                               error bound, exact round trip of {0, +-amax}); the FORMAT itself
 //                               (granularity, amax/448) is reading R10/R11 — the paper only says
@@ -173,6 +176,64 @@ int64_t oracle_mask_to_index_64x128(const uint32_t* bitmask, int L, int H, int N
                         if (64 * t >= N) continue;
                         if (col_idx)
                             col_idx[nnz] = static_cast<uint32_t>(t) | (ku ? 0u : 1u << 30) | (kl ? 0u : 1u << 31);
+                        ++nnz;
+                    }
+                }
+                row_ptr[R + 1] = static_cast<int32_t>(nnz);
+            }
+    return nnz;
+}
+
+// -------------------------------------------------------------------------------------------------
+// f-4  The same two decodes with 16-bit entries (SURVEY section 8 f-4 "uint16 col_idx"; the index is
+// what the mask decode writes and the attention kernel reads, "loaded and used
+// directly": at 25 % density the entries are 5.24 of the 5.9 MB a 480p layer's decode moves, and a
+// key-block index of the paper's shapes (512 / 1182) fits 16 bits).  Written out on their own, one
+// bit at a time like the 32-bit forms.  Plain geometry: entry = kb, nk <= 65536.  64 x 128 geometry:
+// entry = t | (upper does not keep kb) << 14 | (lower does not keep kb) << 15, tiles t < 16384.
+// Return -1 (nothing written) when an index does not fit.
+// -------------------------------------------------------------------------------------------------
+int64_t oracle_mask_to_index_u16(const uint32_t* bitmask, int L, int H, int nq, int nk,
+                                 int32_t* row_ptr, uint16_t* col_idx) {
+    if (nk > 65536) return -1;
+    const int words = (nk + 31) / 32;
+    int64_t nnz = 0, r = 0;
+    row_ptr[0] = 0;
+    for (int l = 0; l < L; ++l)
+        for (int h = 0; h < H; ++h)
+            for (int qb = 0; qb < nq; ++qb, ++r) {
+                for (int kb = 0; kb < nk; ++kb) {
+                    const uint32_t word = bitmask[r * words + kb / 32];
+                    if ((word >> (kb % 32)) & 1u) {
+                        if (col_idx) col_idx[nnz] = static_cast<uint16_t>(kb);
+                        ++nnz;
+                    }
+                }
+                row_ptr[r + 1] = static_cast<int32_t>(nnz);
+            }
+    return nnz;
+}
+
+int64_t oracle_mask_to_index_64x128_u16(const uint32_t* bitmask, int L, int H, int N,
+                                        int32_t* row_ptr, uint16_t* col_idx) {
+    const int nq64 = (N + 63) / 64, nk128 = (N + 127) / 128, nq128 = (N + 127) / 128;
+    if ((N + 63) / 64 > 16384) return -1;
+    const int words = (nk128 + 31) / 32;
+    int64_t nnz = 0, R = 0;
+    row_ptr[0] = 0;
+    for (int l = 0; l < L; ++l)
+        for (int h = 0; h < H; ++h)
+            for (int qb = 0; qb < nq128; ++qb, ++R) {
+                const int64_t upper = ((static_cast<int64_t>(l) * H + h) * nq64 + 2 * qb) * words;
+                const bool has_lower = 2 * qb + 1 < nq64;
+                for (int kb = 0; kb < nk128; ++kb) {
+                    const bool ku = (bitmask[upper + kb / 32] >> (kb % 32)) & 1u;
+                    const bool kl = has_lower && ((bitmask[upper + words + kb / 32] >> (kb % 32)) & 1u);
+                    if (!ku && !kl) continue;
+                    for (int t = 2 * kb; t <= 2 * kb + 1; ++t) {
+                        if (64 * t >= N) continue;
+                        if (col_idx)
+                            col_idx[nnz] = static_cast<uint16_t>(t | (ku ? 0 : 1 << 14) | (kl ? 0 : 1 << 15));
                         ++nnz;
                     }
                 }

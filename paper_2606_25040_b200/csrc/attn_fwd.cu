@@ -17,19 +17,16 @@
 //                 from pair j to pair j+1 through shared memory and a 64-thread named barrier
 //                 (arrive after the max pass of pair j, sync before the exp pass of pair j+1).
 // The 128 scores of a row are streamed from tensor memory twice, 32 columns at a time (max pass,
-// then exp pass), so only 64 are live in registers.  P (bf16 / e4m3) overwrites the first columns of
+// then exp pass), so only 64 are live in registers.  P (bf16 / fp16) overwrites the first columns of
 // its S buffer behind the read position.  O (fp32, 128 TMEM columns) is rescaled lazily: only when a
-// row max grows by more than 2^8 (2^3 for FP8) over m_ref.  The epilogue adds the two warps' partial
+// row max grows by more than 2^8 over m_ref.  The epilogue adds the two warps' partial
 // row sums, normalises, converts to bf16, stages in shared memory and writes with TMA stores
 // (coalesced 128-byte rows; rows beyond N are clipped by the tensor map).
 //
 // FP16 variant (template kF16; "for the non-quantized (fp16) path"): fp16 Q / K / V, P
 // and O; the same pipeline with the kind::f16 operand format switched.
 //
-// FP8 variant (template kFp8; R10-R12): e4m3 Q / K / V tiles (one 128-byte row holds all
-// 128 channels), tcgen05.mma kind::f8f6f4 with fp32 accumulation, V again an MN-major B operand,
-// P cast to e4m3 after a 2^5 shift, the Q / K block scales folded into the exp2 constant of each
-// 64-key tile and V's per-channel scale applied in the epilogue.
+// The FP8 (e4m3) path is a kernel of its own: attn_fwd_fp8.cu.
 #include <cuda_bf16.h>
 
 #include "attn_common.cuh"
@@ -42,14 +39,13 @@ using namespace attn;
 
 constexpr int SBUFS = 3;
 
-// Per-dtype geometry.  A "slab" is a [128 rows][128 B] swizzled tile: 64 bf16 channels or all 128
-// e4m3 channels of 128 rows (one Q block, or the two 64-key tiles of a pair).
-template <bool kFp8>
+// Geometry.  A "slab" is a [128 rows][128 B] swizzled tile: 64 of the 128 channels of 128 rows (one Q
+// block, or the two 64-key tiles of a pair).
 struct Cfg {
-    static constexpr uint32_t SLABS = kFp8 ? 1 : 2;                 // slabs per 128-row, 128-channel tile
+    static constexpr uint32_t SLABS = 2;                            // slabs per 128-row, 128-channel tile
     static constexpr uint32_t TILE_BYTES = SLABS * 16384;           // Q block, or one K / V pair stage
     static constexpr uint32_t HALF_BYTES = 8192;                    // second tile of a pair inside a slab
-    static constexpr int KSTAGES = kFp8 ? 4 : 2, VSTAGES = kFp8 ? 4 : 3;
+    static constexpr int KSTAGES = 2, VSTAGES = 3;
     // shared memory map (bytes from a 1024-aligned base)
     static constexpr uint32_t SQ_OFF = 0;
     static constexpr uint32_t SK_OFF = TILE_BYTES;
@@ -65,17 +61,10 @@ struct Cfg {
         B_O_FREE = B_ITEM_DONE + 1, B_COUNT = B_O_FREE + 1;
     static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
     static_assert(B_COUNT * 8 + 8 <= 256, "barrier area too small");
-    // P: exp2(x - m_ref + P_SHIFT).  bf16 keeps P <= 2^8 under the lazy threshold; e4m3 (max 448,
-    // smallest normal 2^-6) shifts P up by 2^5 and tightens the threshold to 2^3 so that P <= 2^8
-    // still holds while probabilities down to 2^-11 of the row maximum stay normal numbers.
-    static constexpr float RESCALE_THRESHOLD = kFp8 ? 3.0f : 8.0f;   // log2 units
-    static constexpr float P_SHIFT = kFp8 ? 5.0f : 0.0f;
-    // which element pairs (index mod 8) take the FMA-pipe polynomial exp2 instead of the MUFU, and
-    // its degree (relative error 7.5e-5 / 1.7e-3, below the bf16 / e4m3 rounding of P)
-    static constexpr uint32_t POLY_MASK = kFp8 ? 0x11u : 0x00u;   // fp8: 2 of every 8 pairs; bf16 / fp16: none (never faster)
-    static constexpr int POLY_DEG = kFp8 ? 2 : 3;
-    // TMEM columns of P per MMA step (16 bf16 keys or 32 e4m3 keys = 8 columns), steps per tile
-    static constexpr int PV_STEPS_PER_TILE = kFp8 ? 2 : 4;
+    // P = exp2(x - m_ref) <= 2^8 under the lazy-rescale threshold of 2^8 (log2 units below)
+    static constexpr float RESCALE_THRESHOLD = 8.0f;
+    // P V steps per 64-key tile: 16 keys (8 TMEM columns of bf16 / fp16 pairs) per MMA
+    static constexpr int PV_STEPS_PER_TILE = 4;
 };
 
 // tensor-memory map (columns): three S buffers (each aliased by its P) and the O accumulator
@@ -88,12 +77,12 @@ constexpr uint32_t NB_PAIR = 1, NB_HALF = 5, NB_HAND = 7;
 // kBeta: first-frame key enhancement (eq. (1)) as a factor on the scores of keys < n_first
 // kHalf: col_idx entries carry per-half flags (bit 30 / 31: query rows 0-63 / 64-127 of the block do NOT keep the
 // tile), as chorus_mask_to_index_64x128 writes them for masks in the paper's 64 x 128 geometry
-template <bool kFp8, bool kF16, bool kBeta, bool kHalf>   // e4m3 inputs / fp16 inputs and output (neither: bf16)
+template <bool kF16, bool kBeta, bool kHalf>   // fp16 inputs and output (else bf16)
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmO,
                 const AttnParams p) {
-    using C = Cfg<kFp8>;
+    using C = Cfg;
     constexpr int KSTAGES = C::KSTAGES, VSTAGES = C::VSTAGES;
     constexpr uint32_t TILE = C::TILE_BYTES, HALF = C::HALF_BYTES;
     // 128-byte swizzle needs a 1024-byte aligned base; the kernel has no static shared memory, so
@@ -146,7 +135,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             // one 128-row, 128-channel box = SLABS loads of [rows][128 B]
             auto load_tile = [&](uint32_t dst, const CUtensorMap* tm, uint32_t b, int row0, int h, int bb) {
                 tma_load_4d(dst, tm, b, 0, row0, h, bb);
-                if constexpr (!kFp8) tma_load_4d(dst + 16384, tm, b, 64, row0, h, bb);
+                tma_load_4d(dst + 16384, tm, b, 64, row0, h, bb);
             };
             uint32_t g = 0, icnt = 0;   // pairs and non-empty items issued so far
             for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
@@ -196,7 +185,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             }
         } else if (warp == MMA_WARP) {
             // kind::f16: format 1 = bf16; kind::f8f6f4: format 0 = e4m3.  PV: B (= V) is MN-major.
-            constexpr uint32_t FMT = (kFp8 || kF16) ? 0u : 1u;   // kind::f16: 0 = fp16, 1 = bf16
+            constexpr uint32_t FMT = kF16 ? 0u : 1u;   // kind::f16: 0 = fp16, 1 = bf16
             constexpr uint32_t IDESC_S128 = make_idesc(FMT, FMT, 128, 128, 0, 0);
             constexpr uint32_t IDESC_S64 = make_idesc(FMT, FMT, 128, 64, 0, 0);
             constexpr uint32_t IDESC_PV = make_idesc(FMT, FMT, 128, 128, 0, 1);   // A and B formats must agree in kind::f16
@@ -219,16 +208,10 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             const uint32_t tS = tmem + TM_S + sb * 128;
                             const uint32_t idesc = two ? IDESC_S128 : IDESC_S64;
                             const uint64_t dKs = dK + ((st * TILE) >> 4);
-                            if constexpr (kFp8) {
 #pragma unroll
-                                for (int ks = 0; ks < 4; ++ks)       // 32 e4m3 channels = 32 B per step
-                                    mma_f8_ss(tS, dQ + ((ks * 32) >> 4), dKs + ((ks * 32) >> 4), idesc, ks > 0);
-                            } else {
-#pragma unroll
-                                for (int ks = 0; ks < 8; ++ks) {     // 16 bf16 channels = 32 B per step, 2 slabs
-                                    const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
-                                    mma_f16_ss(tS, dQ + off, dKs + off, idesc, ks > 0);
-                                }
+                            for (int ks = 0; ks < 8; ++ks) {     // 16 channels = 32 B per step, 2 slabs
+                                const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
+                                mma_f16_ss(tS, dQ + off, dKs + off, idesc, ks > 0);
                             }
                             tc_commit(bar(C::B_K_EMPTY + st));
                             tc_commit(bar(C::B_S_FULL + sb));
@@ -248,19 +231,17 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         if (elect_one()) {
                             const uint32_t tP = tmem + TM_S + sb * 128, tO = tmem + TM_O;
                             const uint64_t dVs = dV + ((st * TILE) >> 4);
-                            constexpr uint32_t KBYTES = kFp8 ? 4096u : 2048u;   // 32 / 16 keys x 128 B per step
+                            constexpr uint32_t KBYTES = 2048u;   // 16 keys x 128 B per step
                             constexpr int STEPS = C::PV_STEPS_PER_TILE;
 #pragma unroll
                             for (int ks = 0; ks < STEPS; ++ks) {
                                 const uint32_t acc = (jp > 0) || (ks > 0);
-                                if constexpr (kFp8) mma_f8_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
-                                else mma_f16_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
+                                mma_f16_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, acc);
                             }
                             if (two) {
 #pragma unroll
                                 for (int ks = STEPS; ks < 2 * STEPS; ++ks) {
-                                    if constexpr (kFp8) mma_f8_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, 1u);
-                                    else mma_f16_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, 1u);
+                                    mma_f16_ts(tO, tP + ks * 8, dVs + ((ks * KBYTES) >> 4), IDESC_PV, 1u);
                                 }
                             }
                             tc_commit(bar(C::B_V_EMPTY + st));
@@ -282,7 +263,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int row = wq * 32 + lane;          // query row inside the block == TMEM lane
         const uint32_t tlane = tmem + (static_cast<uint32_t>(wq * 32) << 16);
         const uint32_t tOs = tlane + TM_O;       // the O accumulator (all 128 columns of this row)
-        const int nsb = (p.N + 127) >> 7;        // FP8: Q/K scale blocks of 128 tokens
         volatile float* xm = xch;                // [128] m_ref hand-off between the two parities
         volatile float* xe = xch + 128;          // [2 parity][m, l][128] epilogue exchange
         uint32_t g0 = 0;                         // pairs of all previous items (S buffer / phase)
@@ -294,15 +274,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             // folded into the exp2 FMA constant.  The key-block indices of the stream's NEXT pair are
             // fetched one pair ahead so that the loads are off the critical path.
             float sl2a = p.scale_log2, sl2b = p.scale_log2;
-            float qsl2 = 0.f;
-            const float* ksc = nullptr;
             int kba_next = 0, kbb_next = 0;
-            if constexpr (kFp8) {
-                const int64_t sbase = (static_cast<int64_t>(it.b) * p.H + it.h) * nsb;
-                qsl2 = p.scale_log2 * __ldg(p.q_scale + sbase + it.qb);
-                ksc = p.k_scale + sbase;
-            }
-            if constexpr (kFp8 || kBeta || kHalf) {
+            if constexpr (kBeta || kHalf) {
                 if (2 * sm < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * sm);
                 if (2 * sm + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * sm + 1);
             }
@@ -311,7 +284,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const uint32_t tS = tlane + TM_S + sb * 128;     // this pair's S, overwritten by its P
                 int va = BK, vb = BK;            // valid keys in the two tiles of the pair
                 int kba = 0, kbb = 0;
-                if constexpr (kFp8 || kBeta || kHalf) {
+                if constexpr (kBeta || kHalf) {
                     kba = kba_next;
                     kbb = kbb_next;
                     if (2 * (j + 2) < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2));
@@ -325,22 +298,18 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     kba &= 0x3fffffff;
                     kbb &= 0x3fffffff;
                 }
-                if constexpr (kFp8) {
-                    sl2a = qsl2 * __ldg(ksc + (kba >> 1));
-                    sl2b = qsl2 * __ldg(ksc + (kbb >> 1));
-                }
                 // kBeta: a tile inside the first frame takes beta in its scale factor; the one tile
                 // that straddles n_first takes it per column (fa / fb leading columns) in the masked body
                 int fa = 0, fb = 0;
                 if constexpr (kBeta) {
-                    if constexpr (!kFp8) sl2a = sl2b = p.scale_log2;
+                    sl2a = sl2b = p.scale_log2;
                     fa = min(BK, max(0, p.n_first - kba * BK));
                     fb = (2 * j + 1 < it.nt) ? min(BK, max(0, p.n_first - kbb * BK)) : 0;
                     if (fa == BK) { sl2a *= p.beta; fa = 0; }
                     if (fb == BK) { sl2b *= p.beta; fb = 0; }
                 }
                 if (j == it.np - 1) {            // only the last pair can be odd or hold the ragged key block
-                    if constexpr (!(kFp8 || kBeta || kHalf)) {
+                    if constexpr (!(kBeta || kHalf)) {
                         kba = __ldg(p.col_idx + it.r0 + 2 * j);
                         if (2 * j + 1 < it.nt) kbb = __ldg(p.col_idx + it.r0 + 2 * j + 1);
                     }
@@ -450,7 +419,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     // pairs whose bit is set in POLY_MASK (index mod 8) take the polynomial exp2 on
                     // the FMA pipe, the rest the MUFU.
                     // kHalf: a row that has kept nothing so far has m_ref = -inf and only -inf scores
-                    const float negm = (kHalf && m_ref == -INFINITY) ? 0.f : C::P_SHIFT - m_ref;
+                    const float negm = (kHalf && m_ref == -INFINITY) ? 0.f : -m_ref;
                     const float2 negm_2 = make_float2(negm, negm);
                     const float2 sl2a_2 = make_float2(sl2a, sl2a), sl2b_2 = make_float2(sl2b, sl2b);
                     float2 lacc = make_float2(l0, l1);
@@ -460,23 +429,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         auto exp_pair = [&](int q) -> float2 {     // q: element pair index 0..15
                             const float2 x = ffma2(make_float2(__uint_as_float(r[2 * q]), __uint_as_float(r[2 * q + 1])),
                                                    sl2_2, negm_2);
-                            if ((C::POLY_MASK >> (q & 7)) & 1u) return exp2_poly2<C::POLY_DEG>(x);
-                            return make_float2(ex2(x.x), ex2(x.y));
+                            return make_float2(ex2(x.x), ex2(x.y));   // all on the MUFU: a polynomial share never paid here
                         };
-                        if constexpr (kFp8) {
-                            // The denominator sums the e4m3-ROUNDED weights (two f16x2 accumulators
-                            // per 32 keys: at most 8 x 2^8 each, exact to 2^-11): exactly what P V uses.
-                            uint32_t pk[8];
-                            uint32_t h0 = 0u, h1 = 0u;
-#pragma unroll
-                            for (int k = 0; k < 8; ++k) {
-                                const float2 pa = exp_pair(2 * k), pb = exp_pair(2 * k + 1);
-                                pk[k] = pack_e4m3x4_acc(pa.x, pa.y, pb.x, pb.y, h0, h1);
-                            }
-                            lacc.x += f16x2_hsum(h0);
-                            lacc.y += f16x2_hsum(h1);
-                            tmem_st8(tS + c * 8, pk);        // P: e4m3 quads over the first 32 S columns
-                        } else {
+                        {
                             uint32_t pk[16];
 #pragma unroll
                             for (int k = 0; k < 16; ++k) {
@@ -527,7 +482,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
                     for (int k = 0; k < 16; ++k) z[k] = 0u;
 #pragma unroll
-                    for (int c = 0; c < (kFp8 ? 2 : 4); ++c) tmem_st16(tS + c * 16, z);
+                    for (int c = 0; c < 4; ++c) tmem_st16(tS + c * 16, z);
                 };
                 if (kHalf && va == 0 && vb == 0) skip_body();
                 else if (ragged) pair_body(BoolTag<true>{});
@@ -559,7 +514,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             // keys; -inf for an empty row): what a later block-mass pass needs
             if (p.lse != nullptr && sm == 0 && it.qb * BQ + row < p.N)
                 p.lse[(static_cast<int64_t>(it.b) * p.H + it.h) * p.N + it.qb * BQ + row] =
-                    (L > 0.f) ? (m_all + lg2(L) - C::P_SHIFT) * 0.6931471805599453f : -INFINITY;
+                    (L > 0.f) ? (m_all + lg2(L)) * 0.6931471805599453f : -INFINITY;
             named_bar_sync(NB_HALF + sm, 128);                 // staging free for the whole warpgroup
             if (it.nt > 0) {
                 mbar_wait(bar(C::B_ITEM_DONE), icnt & 1);      // every P V of the item has completed
@@ -567,10 +522,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             }
             const uint32_t srow = sO + sm * 16384 + row * 128;
             const uint32_t tO = tOs + sm * 64;
-            // FP8: O[:, c] carries V's per-channel scale (R10)
-            const float4* vsc = nullptr;
-            if constexpr (kFp8)
-                vsc = reinterpret_cast<const float4*>(p.v_scale + (static_cast<int64_t>(it.b) * p.H + it.h) * 128 + sm * 64);
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
                 uint32_t o[32];
@@ -581,11 +532,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 uint32_t pk[16];
 #pragma unroll
                 for (int k4 = 0; k4 < 8; ++k4) {
-                    float4 w = make_float4(inv, inv, inv, inv);
-                    if constexpr (kFp8) {
-                        const float4 sc = __ldg(vsc + c * 8 + k4);
-                        w = make_float4(inv * sc.x, inv * sc.y, inv * sc.z, inv * sc.w);
-                    }
+                    const float4 w = make_float4(inv, inv, inv, inv);
                     float x0 = 0.f, x1 = 0.f, x2 = 0.f, x3 = 0.f;
                     if (it.nt > 0) {
                         x0 = __uint_as_float(o[4 * k4]) * w.x;     x1 = __uint_as_float(o[4 * k4 + 1]) * w.y;
@@ -624,18 +571,18 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 }  // namespace
 
-template <bool kFp8, bool kF16, bool kBeta, bool kHalf>
+template <bool kF16, bool kBeta, bool kHalf>
 static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                               const CUtensorMap& tmO, const AttnParams& p, cudaStream_t stream) {
-    constexpr uint32_t smem = Cfg<kFp8>::SMEM_BYTES;
-    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kFp8, kF16, kBeta, kHalf>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    constexpr uint32_t smem = Cfg::SMEM_BYTES;
+    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<kF16, kBeta, kHalf>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     const int n_items = p.B * p.H * p.nq;
     const int grid = n_items < sms ? n_items : sms;
-    attn_fwd_kernel<kFp8, kF16, kBeta, kHalf><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
+    attn_fwd_kernel<kF16, kBeta, kHalf><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
     count_launch(1);
     return cudaGetLastError();
 }
@@ -644,16 +591,16 @@ cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, cons
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
                             cudaStream_t stream) {
     const bool beta = p.n_first > 0 && p.beta != 1.f;
-    auto go = [&](auto fp8, auto f16) -> cudaError_t {
-        constexpr bool F8 = decltype(fp8)::value, F16 = decltype(f16)::value;
-        if (beta && p.half_flags) return launch_one<F8, F16, true, true>(tmQ, tmK, tmV, tmO, p, stream);
-        if (beta) return launch_one<F8, F16, true, false>(tmQ, tmK, tmV, tmO, p, stream);
-        if (p.half_flags) return launch_one<F8, F16, false, true>(tmQ, tmK, tmV, tmO, p, stream);
-        return launch_one<F8, F16, false, false>(tmQ, tmK, tmV, tmO, p, stream);
+    auto go = [&](auto f16) -> cudaError_t {
+        constexpr bool F16 = decltype(f16)::value;
+        if (beta && p.half_flags) return launch_one<F16, true, true>(tmQ, tmK, tmV, tmO, p, stream);
+        if (beta) return launch_one<F16, true, false>(tmQ, tmK, tmV, tmO, p, stream);
+        if (p.half_flags) return launch_one<F16, false, true>(tmQ, tmK, tmV, tmO, p, stream);
+        return launch_one<F16, false, false>(tmQ, tmK, tmV, tmO, p, stream);
     };
-    if (dtype == CHORUS_BF16) return go(BoolTag<false>{}, BoolTag<false>{});
-    if (dtype == CHORUS_FP8_E4M3) return launch_attn_fwd_fp8(tmQ, tmK, tmV, tmO, p, stream);
-    if (dtype == CHORUS_FP16) return go(BoolTag<false>{}, BoolTag<true>{});
+    if (dtype == CHORUS_BF16) return go(BoolTag<false>{});
+    if (dtype == CHORUS_FP8_E4M3) return launch_attn_fwd_fp8(tmQ, tmK, tmV, tmO, p, stream);   // attn_fwd_fp8.cu
+    if (dtype == CHORUS_FP16) return go(BoolTag<true>{});
     return cudaErrorNotSupported;
 }
 

@@ -245,13 +245,6 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
         "r"(r[15])
         : "memory");
 }
-__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* r) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
-        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]),
-        "r"(r[7])
-        : "memory");
-}
 
 __device__ __forceinline__ float ex2(float x) {
     float y;
@@ -333,34 +326,6 @@ __device__ __forceinline__ uint32_t pack_e4m3x4(float a, float b, float c, float
         : "=r"(r)
         : "f"(a), "f"(b), "f"(c), "f"(d));
     return r;
-}
-
-// The same, and the four ROUNDED values are added to two f16x2 accumulators (acc0 += {a^, b^},
-// acc1 += {c^, d^}): the softmax denominator is then the sum of exactly the weights the P V
-// product uses, so a row dominated by one key is reproduced without the e4m3 rounding of its weight.
-__device__ __forceinline__ uint32_t pack_e4m3x4_acc(float a, float b, float c, float d,
-                                                    uint32_t& acc0, uint32_t& acc1) {
-    uint32_t r;
-    asm("{\n\t.reg .b16 lo, hi;\n\t.reg .b32 h0, h1;\n\t"
-        "cvt.rn.satfinite.e4m3x2.f32 lo, %4, %3;\n\t"
-        "cvt.rn.satfinite.e4m3x2.f32 hi, %6, %5;\n\t"
-        "mov.b32 %0, {lo, hi};\n\t"
-        "cvt.rn.f16x2.e4m3x2 h0, lo;\n\t"
-        "cvt.rn.f16x2.e4m3x2 h1, hi;\n\t"
-        "add.rn.f16x2 %1, %1, h0;\n\t"
-        "add.rn.f16x2 %2, %2, h1;\n\t}\n"
-        : "=r"(r), "+r"(acc0), "+r"(acc1)
-        : "f"(a), "f"(b), "f"(c), "f"(d));
-    return r;
-}
-// sum of the two halves of an f16x2 register, as fp32
-__device__ __forceinline__ float f16x2_hsum(uint32_t h) {
-    float lo, hi;
-    asm("{\n\t.reg .b16 a, b;\n\tmov.b32 {a, b}, %2;\n\t"
-        "cvt.f32.f16 %0, a;\n\tcvt.f32.f16 %1, b;\n\t}\n"
-        : "=f"(lo), "=f"(hi)
-        : "r"(h));
-    return lo + hi;
 }
 
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
