@@ -217,6 +217,39 @@ chorus_status chorus_block_sparse_attn_fwd_64x128(const void* Q, const void* K, 
                                                   int n_first, float beta, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * 16-bit index entries (the decoded index is what the attention
+ * kernel "loads and uses directly", and at 25 % density its entries are 5.24 of the 5.9 MB that the
+ * decode of a 480p layer moves: 16-bit entries halve that, and the key-block indices of the
+ * paper's shapes, 512 and 1182, fit).
+ *
+ * chorus_mask_to_index_u16, chorus_mask_to_index_64x128_u16: the two decodes above with
+ *   col_idx   device, uint16 [col_cap] (2-byte aligned) or NULL (count only).  Plain geometry: the
+ *             key-block index (nk_blk <= 65536).  64 x 128 geometry: t | (upper does not keep kb) << 14
+ *             | (lower does not keep kb) << 15 (ceil(N/64) <= 16384).
+ *   row_ptr, workspace, order of the entries: exactly as in the 32-bit calls; compared bit-exactly
+ *   with the oracle's 16-bit forms.
+ * chorus_block_sparse_attn_fwd_idx16: the attention call on such an index.  Arguments as
+ *   chorus_block_sparse_attn_fwd_first_frame plus geometry_64x128 (non-zero: the entries carry the two
+ *   per-half flags, as chorus_block_sparse_attn_fwd_64x128 takes them in 32 bits).  The result is
+ *   bit-identical to the call on the 32-bit index of the same mask.
+ * Errors: as the 32-bit calls, and UNSUPPORTED when an index does not fit (nk_blk > 65536, or more
+ *         than 16384 tiles with the flags).
+ * ------------------------------------------------------------------------------------------- */
+chorus_status chorus_mask_to_index_u16(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                       int32_t* row_ptr, uint16_t* col_idx, int64_t col_cap,
+                                       void* workspace, size_t* workspace_bytes, void* cuda_stream);
+chorus_status chorus_mask_to_index_64x128_u16(const uint32_t* bitmask, int L, int H, int N,
+                                              int32_t* row_ptr, uint16_t* col_idx, int64_t col_cap,
+                                              void* workspace, size_t* workspace_bytes, void* cuda_stream);
+chorus_status chorus_block_sparse_attn_fwd_idx16(const void* Q, const void* K, const void* V,
+                                                 const int32_t* row_ptr, const uint16_t* col_idx,
+                                                 float scale, chorus_dtype dtype, void* O,
+                                                 const chorus_attn_shape* shape,
+                                                 const chorus_fp8_scales* fp8, float* lse,
+                                                 int n_first, float beta, int geometry_64x128,
+                                                 void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * FP8 quantisation pre-pass for dtype = CHORUS_FP8_E4M3 (PAPER.md:L97 says only "FP8
  * quantization"; granularity and formula are BASELINE.json configs[2] / DESIGN.md R10-R11):
  *     s  = max(amax, 1e-12) / 448      x8 = e4m3_rne_saturate(x / s)       (fp32 arithmetic)

@@ -21,6 +21,7 @@ BLOCK_Q, BLOCK_K, HEAD_DIM = 128, 64, 128
 EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_attn_fwd",
            "chorus_block_sparse_attn_fwd_lse", "chorus_block_sparse_attn_fwd_first_frame",
            "chorus_mask_to_index_64x128", "chorus_block_sparse_attn_fwd_64x128", "chorus_block_mass_64x128",
+           "chorus_mask_to_index_u16", "chorus_mask_to_index_64x128_u16", "chorus_block_sparse_attn_fwd_idx16",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
            "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_gather_heads", "chorus_scatter_heads", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count", "chorus_tensor_map_encodes"]
@@ -81,6 +82,10 @@ def lib() -> C.CDLL:
         L.chorus_block_sparse_attn_fwd_64x128.argtypes = L.chorus_block_sparse_attn_fwd_first_frame.argtypes
         L.chorus_mask_to_index_64x128.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                                   C.c_int64, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p]
+        L.chorus_mask_to_index_u16.argtypes = L.chorus_mask_to_index.argtypes
+        L.chorus_mask_to_index_64x128_u16.argtypes = L.chorus_mask_to_index_64x128.argtypes
+        L.chorus_block_sparse_attn_fwd_idx16.argtypes = (
+            L.chorus_block_sparse_attn_fwd_first_frame.argtypes[:-1] + [C.c_int, C.c_void_p])
         L.chorus_mask_from_mass.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double,
                                             C.c_void_p, C.c_void_p, C.c_void_p]
         L.chorus_mask_coverage.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
@@ -131,8 +136,9 @@ def mask_to_index_workspace_bytes(L: int, H: int, nq_blk: int, nk_blk: int) -> i
 
 
 def chorus_mask_to_index(bitmask, nk_blk: int, row_ptr=None, col_idx=None, workspace=None,
-                         stream=None, count_only=False):
+                         stream=None, count_only=False, idx16=False):
     """bitmask: cuda int32/uint32-bits tensor [L][H][nq][words].  Returns (row_ptr, col_idx).
+    idx16 (or a 2-byte col_idx tensor): 16-bit entries (chorus_mask_to_index_u16).
 
     If col_idx is not given: count-only pass, one 4-byte read of nnz, allocation, second pass
     (the protocol include/chorus.h describes)."""
@@ -147,20 +153,23 @@ def chorus_mask_to_index(bitmask, nk_blk: int, row_ptr=None, col_idx=None, works
         workspace = torch.empty(max(mask_to_index_workspace_bytes(L, H, nq, nk_blk), 4),
                                 dtype=torch.uint8, device=dev)
     wsb = C.c_size_t(workspace.numel())
+    idx16 = idx16 or (col_idx is not None and col_idx.element_size() == 2)
+    fn = lib().chorus_mask_to_index_u16 if idx16 else lib().chorus_mask_to_index
     if col_idx is None:
-        _check(lib().chorus_mask_to_index(_ptr(bitmask), L, H, nq, nk_blk, _ptr(row_ptr), None, 0,
-                                          _ptr(workspace), C.byref(wsb), _stream(stream)))
+        _check(fn(_ptr(bitmask), L, H, nq, nk_blk, _ptr(row_ptr), None, 0,
+                  _ptr(workspace), C.byref(wsb), _stream(stream)))
         if count_only:
             return row_ptr, None
         nnz = int(row_ptr[-1].item())
-        col_idx = torch.empty(max(nnz, 1), dtype=torch.int32, device=dev)
-    _check(lib().chorus_mask_to_index(_ptr(bitmask), L, H, nq, nk_blk, _ptr(row_ptr), _ptr(col_idx),
-                                      col_idx.numel(), _ptr(workspace), C.byref(wsb), _stream(stream)))
+        col_idx = torch.empty(max(nnz, 1), dtype=torch.uint16 if idx16 else torch.int32, device=dev)
+    assert col_idx.element_size() == (2 if idx16 else 4)
+    _check(fn(_ptr(bitmask), L, H, nq, nk_blk, _ptr(row_ptr), _ptr(col_idx),
+              col_idx.numel(), _ptr(workspace), C.byref(wsb), _stream(stream)))
     return row_ptr, col_idx
 
 
 def chorus_mask_to_index_64x128(bitmask, N: int, row_ptr=None, col_idx=None, workspace=None, stream=None,
-                                count_only=False):
+                                count_only=False, idx16=False):
     """bitmask: cuda 4-byte tensor [L][H][ceil(N/64)][words] in the paper's 64 x 128 geometry.  Returns
     (row_ptr [L*H*ceil(N/128)+1], col_idx with the per-half flag bits) for chorus_block_sparse_attn_fwd(...,
     geometry_64x128=True).  Same two-pass protocol as chorus_mask_to_index."""
@@ -175,14 +184,16 @@ def chorus_mask_to_index_64x128(bitmask, N: int, row_ptr=None, col_idx=None, wor
         _check(lib().chorus_mask_to_index_64x128(None, L, H, N, None, None, 0, None, C.byref(need), None))
         workspace = torch.empty(max(need.value, 16), dtype=torch.uint8, device=dev)
     wsb = C.c_size_t(workspace.numel())
+    idx16 = idx16 or (col_idx is not None and col_idx.element_size() == 2)
+    fn = lib().chorus_mask_to_index_64x128_u16 if idx16 else lib().chorus_mask_to_index_64x128
     if col_idx is None:
-        _check(lib().chorus_mask_to_index_64x128(_ptr(bitmask), L, H, N, _ptr(row_ptr), None, 0,
-                                                 _ptr(workspace), C.byref(wsb), _stream(stream)))
+        _check(fn(_ptr(bitmask), L, H, N, _ptr(row_ptr), None, 0, _ptr(workspace), C.byref(wsb), _stream(stream)))
         if count_only:
             return row_ptr, None
-        col_idx = torch.empty(max(int(row_ptr[-1].item()), 1), dtype=torch.int32, device=dev)
-    _check(lib().chorus_mask_to_index_64x128(_ptr(bitmask), L, H, N, _ptr(row_ptr), _ptr(col_idx),
-                                             col_idx.numel(), _ptr(workspace), C.byref(wsb), _stream(stream)))
+        col_idx = torch.empty(max(int(row_ptr[-1].item()), 1), dtype=torch.uint16 if idx16 else torch.int32, device=dev)
+    assert col_idx.element_size() == (2 if idx16 else 4)
+    _check(fn(_ptr(bitmask), L, H, N, _ptr(row_ptr), _ptr(col_idx),
+              col_idx.numel(), _ptr(workspace), C.byref(wsb), _stream(stream)))
     return row_ptr, col_idx
 
 
@@ -226,6 +237,13 @@ def chorus_block_sparse_attn_fwd(Q, K, V, row_ptr, col_idx, scale: float, dtype:
         sc = Fp8Scales(*(x.data_ptr() for x in fp8_scales))
     if lse is not None:     # float32 [B][H][N], written by the kernel (natural-log row log-sum-exp)
         assert lse.dtype == torch.float32 and lse.is_contiguous() and lse.shape == (B, H, N)
+    if col_idx.element_size() == 2:     # 16-bit index entries (chorus_mask_to_index_u16 / _64x128_u16)
+        _check(lib().chorus_block_sparse_attn_fwd_idx16(
+            _ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx), C.c_float(scale), dtype, _ptr(O),
+            C.byref(shape), C.byref(sc) if sc is not None else None,
+            _ptr(lse) if lse is not None else None, C.c_int(int(n_first)), C.c_float(float(beta)),
+            C.c_int(int(bool(geometry_64x128))), _stream(stream)))
+        return O
     if geometry_64x128:
         _check(lib().chorus_block_sparse_attn_fwd_64x128(
             _ptr(Q), _ptr(K), _ptr(V), _ptr(row_ptr), _ptr(col_idx), C.c_float(scale), dtype, _ptr(O),

@@ -21,6 +21,14 @@ struct BoolTag {
     static constexpr bool value = V;
 };
 
+// entry i of the index in its 32-bit form, whichever width it is stored in: a 16-bit entry is zero-extended, and
+// its two per-half flags (bits 14 / 15, 64 x 128 geometry) go to bits 30 / 31
+__device__ __forceinline__ int ld_col(const AttnParams& p, int64_t i) {
+    if (!p.idx16) return __ldg(static_cast<const int32_t*>(p.col_idx) + i);
+    const uint32_t e = __ldg(static_cast<const uint16_t*>(p.col_idx) + i);
+    return p.half_flags ? static_cast<int>((e & 0x3fffu) | ((e >> 14) << 30)) : static_cast<int>(e);
+}
+
 struct Item {
     int b, h, qb, r0, nt, np;
 };

@@ -150,7 +150,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 // the key-block indices of 16 pairs are fetched with one coalesced load
                 for (int j0 = 0; j0 < it.np; j0 += 16) {
                     const int t = 2 * j0 + lane;
-                    int mine = (t < it.nt) ? __ldg(p.col_idx + it.r0 + t) : 0;
+                    int mine = (t < it.nt) ? ld_col(p, it.r0 + t) : 0;
                     if constexpr (kHalf) mine &= 0x3fffffff;
                     const int jn = min(16, it.np - j0);
                     for (int jl = 0; jl < jn; ++jl, ++g) {
@@ -276,8 +276,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             float sl2a = p.scale_log2, sl2b = p.scale_log2;
             int kba_next = 0, kbb_next = 0;
             if constexpr (kBeta || kHalf) {
-                if (2 * sm < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * sm);
-                if (2 * sm + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * sm + 1);
+                if (2 * sm < it.nt) kba_next = ld_col(p, it.r0 + 2 * sm);
+                if (2 * sm + 1 < it.nt) kbb_next = ld_col(p, it.r0 + 2 * sm + 1);
             }
             for (int j = sm; j < it.np; j += 2) {
                 const uint32_t g = g0 + j, sb = g % SBUFS;
@@ -287,8 +287,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 if constexpr (kBeta || kHalf) {
                     kba = kba_next;
                     kbb = kbb_next;
-                    if (2 * (j + 2) < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2));
-                    if (2 * (j + 2) + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2) + 1);
+                    if (2 * (j + 2) < it.nt) kba_next = ld_col(p, it.r0 + 2 * (j + 2));
+                    if (2 * (j + 2) + 1 < it.nt) kbb_next = ld_col(p, it.r0 + 2 * (j + 2) + 1);
                 }
                 uint32_t skip_a = 0u, skip_b = 0u;   // kHalf: this warp's rows do not keep tile a / b
                 if constexpr (kHalf) {
@@ -310,8 +310,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 }
                 if (j == it.np - 1) {            // only the last pair can be odd or hold the ragged key block
                     if constexpr (!(kBeta || kHalf)) {
-                        kba = __ldg(p.col_idx + it.r0 + 2 * j);
-                        if (2 * j + 1 < it.nt) kbb = __ldg(p.col_idx + it.r0 + 2 * j + 1);
+                        kba = ld_col(p, it.r0 + 2 * j);
+                        if (2 * j + 1 < it.nt) kbb = ld_col(p, it.r0 + 2 * j + 1);
                     }
                     va = min(BK, p.N - kba * BK);
                     vb = (2 * j + 1 < it.nt) ? min(BK, p.N - kbb * BK) : 0;

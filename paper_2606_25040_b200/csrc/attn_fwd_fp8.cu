@@ -126,7 +126,7 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                 // the key-block indices of 16 pairs are fetched with one coalesced load
                 for (int j0 = 0; j0 < it.np; j0 += 16) {
                     const int t = 2 * j0 + lane;
-                    int mine = (t < it.nt) ? __ldg(p.col_idx + it.r0 + t) : 0;
+                    int mine = (t < it.nt) ? ld_col(p, it.r0 + t) : 0;
                     if constexpr (kHalf) mine &= 0x3fffffff;
                     const int jn = min(16, it.np - j0);
                     for (int jl = 0; jl < jn; ++jl, ++g) {
@@ -243,15 +243,15 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
             const float qsl2 = p.scale_log2 * __ldg(p.q_scale + sbase + it.qb);
             const float* ksc = p.k_scale + sbase;
             int kba_next = 0, kbb_next = 0;
-            if (2 * sm < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * sm);
-            if (2 * sm + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * sm + 1);
+            if (2 * sm < it.nt) kba_next = ld_col(p, it.r0 + 2 * sm);
+            if (2 * sm + 1 < it.nt) kbb_next = ld_col(p, it.r0 + 2 * sm + 1);
             for (int j = sm; j < it.np; j += 2) {
                 const uint32_t g = g0 + j, sb = g % SBUFS, pb = g % PBUFS;
                 const uint32_t tS = tlane + TM_S + sb * 128, tP = tlane + TM_P + pb * 32;
                 int va = BK, vb = BK;            // valid keys in the two tiles of the pair
                 int kba = kba_next, kbb = kbb_next;
-                if (2 * (j + 2) < it.nt) kba_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2));
-                if (2 * (j + 2) + 1 < it.nt) kbb_next = __ldg(p.col_idx + it.r0 + 2 * (j + 2) + 1);
+                if (2 * (j + 2) < it.nt) kba_next = ld_col(p, it.r0 + 2 * (j + 2));
+                if (2 * (j + 2) + 1 < it.nt) kbb_next = ld_col(p, it.r0 + 2 * (j + 2) + 1);
                 uint32_t skip_a = 0u, skip_b = 0u;   // kHalf: this warp's rows do not keep tile a / b
                 if constexpr (kHalf) {
                     const int hb = 30 + (wq >> 1);

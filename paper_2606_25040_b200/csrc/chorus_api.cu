@@ -139,14 +139,16 @@ int64_t chorus_launch_count(void) { return g_launches; }
 int64_t chorus_tensor_map_encodes(void) { return g_tmap_encodes; }
 void chorus_reset_launch_count(void) { g_launches = 0; }
 
-chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
-                                   int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
-                                   void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+static chorus_status mask_to_index_impl(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                        int32_t* row_ptr, void* col_idx, bool idx16, int64_t col_cap,
+                                        void* workspace, size_t* workspace_bytes, void* cuda_stream) {
     g_err[0] = 0;
     if (!workspace_bytes) return set_error(CHORUS_ERR_INVALID_ARG, "workspace_bytes is null");
     if (L <= 0 || H <= 0 || nq_blk <= 0 || nk_blk <= 0)
         return set_error(CHORUS_ERR_INVALID_ARG, "L, H, nq_blk, nk_blk must be positive (%d %d %d %d)",
                          L, H, nq_blk, nk_blk);
+    if (idx16 && nk_blk > 65536)
+        return set_error(CHORUS_ERR_UNSUPPORTED, "nk_blk = %d does not fit a 16-bit index", nk_blk);
     const int64_t rows = static_cast<int64_t>(L) * H * nq_blk;
     if (rows * nk_blk > INT32_MAX)
         return set_error(CHORUS_ERR_CAPACITY, "L*H*nq_blk*nk_blk = %lld exceeds INT32_MAX",
@@ -159,25 +161,43 @@ chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq
     if (!bitmask || !row_ptr) return set_error(CHORUS_ERR_INVALID_ARG, "bitmask / row_ptr is null");
     if (col_cap < 0) return set_error(CHORUS_ERR_INVALID_ARG, "col_cap < 0");
     if ((reinterpret_cast<uintptr_t>(bitmask) | reinterpret_cast<uintptr_t>(row_ptr) |
-         reinterpret_cast<uintptr_t>(col_idx) | reinterpret_cast<uintptr_t>(workspace)) & 3u)
+         reinterpret_cast<uintptr_t>(workspace)) & 3u)
         return set_error(CHORUS_ERR_INVALID_ARG, "pointers must be 4-byte aligned");
+    if (reinterpret_cast<uintptr_t>(col_idx) & (idx16 ? 1u : 3u))
+        return set_error(CHORUS_ERR_INVALID_ARG, "col_idx must be aligned to its entry size");
     if (*workspace_bytes < need)
         return set_error(CHORUS_ERR_CAPACITY, "workspace too small: %zu < %zu", *workspace_bytes, need);
     const int words = (nk_blk + 31) / 32;
-    return check_cuda(launch_mask_decode(bitmask, rows, nk_blk, words, row_ptr, col_idx, col_cap,
+    return check_cuda(launch_mask_decode(bitmask, rows, nk_blk, words, row_ptr, col_idx, idx16, col_cap,
                                          workspace, static_cast<cudaStream_t>(cuda_stream)),
                       "mask decode launch");
 }
 
-chorus_status chorus_mask_to_index_64x128(const uint32_t* bitmask, int L, int H, int N,
-                                          int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
-                                          void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                   int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
+                                   void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+    return mask_to_index_impl(bitmask, L, H, nq_blk, nk_blk, row_ptr, col_idx, false, col_cap, workspace,
+                              workspace_bytes, cuda_stream);
+}
+
+chorus_status chorus_mask_to_index_u16(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                       int32_t* row_ptr, uint16_t* col_idx, int64_t col_cap,
+                                       void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+    return mask_to_index_impl(bitmask, L, H, nq_blk, nk_blk, row_ptr, col_idx, true, col_cap, workspace,
+                              workspace_bytes, cuda_stream);
+}
+
+static chorus_status mask_to_index_64x128_impl(const uint32_t* bitmask, int L, int H, int N,
+                                               int32_t* row_ptr, void* col_idx, bool idx16, int64_t col_cap,
+                                               void* workspace, size_t* workspace_bytes, void* cuda_stream) {
     g_err[0] = 0;
     if (!workspace_bytes) return set_error(CHORUS_ERR_INVALID_ARG, "workspace_bytes is null");
     if (L <= 0 || H <= 0 || N <= 0)
         return set_error(CHORUS_ERR_INVALID_ARG, "L, H, N must be positive (%d %d %d)", L, H, N);
     const int64_t heads = static_cast<int64_t>(L) * H;
     const int64_t nq128 = (static_cast<int64_t>(N) + 127) / 128, nk64 = (static_cast<int64_t>(N) + 63) / 64;
+    if (idx16 && nk64 > 16384)
+        return set_error(CHORUS_ERR_UNSUPPORTED, "%lld tiles do not fit a 14-bit index", static_cast<long long>(nk64));
     if (heads * nq128 * nk64 > INT32_MAX)
         return set_error(CHORUS_ERR_CAPACITY, "L*H*ceil(N/128)*ceil(N/64) = %lld exceeds INT32_MAX",
                          static_cast<long long>(heads * nq128 * nk64));
@@ -188,16 +208,31 @@ chorus_status chorus_mask_to_index_64x128(const uint32_t* bitmask, int L, int H,
     }
     if (!bitmask || !row_ptr) return set_error(CHORUS_ERR_INVALID_ARG, "bitmask / row_ptr is null");
     if (col_cap < 0) return set_error(CHORUS_ERR_INVALID_ARG, "col_cap < 0");
-    if ((reinterpret_cast<uintptr_t>(bitmask) | reinterpret_cast<uintptr_t>(row_ptr) |
-         reinterpret_cast<uintptr_t>(col_idx)) & 3u)
+    if ((reinterpret_cast<uintptr_t>(bitmask) | reinterpret_cast<uintptr_t>(row_ptr)) & 3u)
         return set_error(CHORUS_ERR_INVALID_ARG, "pointers must be 4-byte aligned");
+    if (reinterpret_cast<uintptr_t>(col_idx) & (idx16 ? 1u : 3u))
+        return set_error(CHORUS_ERR_INVALID_ARG, "col_idx must be aligned to its entry size");
     if (reinterpret_cast<uintptr_t>(workspace) & 15u)
         return set_error(CHORUS_ERR_INVALID_ARG, "workspace must be 16-byte aligned");
     if (*workspace_bytes < need)
         return set_error(CHORUS_ERR_CAPACITY, "workspace too small: %zu < %zu", *workspace_bytes, need);
-    return check_cuda(launch_mask_decode_64x128(bitmask, heads, N, row_ptr, col_idx, col_cap, workspace,
+    return check_cuda(launch_mask_decode_64x128(bitmask, heads, N, row_ptr, col_idx, idx16, col_cap, workspace,
                                                 static_cast<cudaStream_t>(cuda_stream)),
                       "64x128 mask decode launch");
+}
+
+chorus_status chorus_mask_to_index_64x128(const uint32_t* bitmask, int L, int H, int N,
+                                          int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
+                                          void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+    return mask_to_index_64x128_impl(bitmask, L, H, N, row_ptr, col_idx, false, col_cap, workspace, workspace_bytes,
+                                     cuda_stream);
+}
+
+chorus_status chorus_mask_to_index_64x128_u16(const uint32_t* bitmask, int L, int H, int N,
+                                              int32_t* row_ptr, uint16_t* col_idx, int64_t col_cap,
+                                              void* workspace, size_t* workspace_bytes, void* cuda_stream) {
+    return mask_to_index_64x128_impl(bitmask, L, H, N, row_ptr, col_idx, true, col_cap, workspace, workspace_bytes,
+                                     cuda_stream);
 }
 
 chorus_status chorus_visit_refresh(uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
@@ -262,7 +297,7 @@ chorus_status chorus_block_sparse_attn_fwd_lse(const void* Q, const void* K, con
 }
 
 static chorus_status attn_impl(const void* Q, const void* K, const void* V, const int32_t* row_ptr,
-                               const int32_t* col_idx, float scale, chorus_dtype dtype, void* O,
+                               const void* col_idx, bool idx16, float scale, chorus_dtype dtype, void* O,
                                const chorus_attn_shape* shape, const chorus_fp8_scales* fp8, float* lse,
                                int n_first, float beta, bool half_flags, void* cuda_stream);
 
@@ -272,7 +307,7 @@ chorus_status chorus_block_sparse_attn_fwd_first_frame(const void* Q, const void
                                                        const chorus_attn_shape* shape,
                                                        const chorus_fp8_scales* fp8, float* lse,
                                                        int n_first, float beta, void* cuda_stream) {
-    return attn_impl(Q, K, V, row_ptr, col_idx, scale, dtype, O, shape, fp8, lse, n_first, beta, false, cuda_stream);
+    return attn_impl(Q, K, V, row_ptr, col_idx, false, scale, dtype, O, shape, fp8, lse, n_first, beta, false, cuda_stream);
 }
 
 chorus_status chorus_block_sparse_attn_fwd_64x128(const void* Q, const void* K, const void* V,
@@ -281,11 +316,22 @@ chorus_status chorus_block_sparse_attn_fwd_64x128(const void* Q, const void* K, 
                                                   const chorus_attn_shape* shape,
                                                   const chorus_fp8_scales* fp8, float* lse,
                                                   int n_first, float beta, void* cuda_stream) {
-    return attn_impl(Q, K, V, row_ptr, col_idx, scale, dtype, O, shape, fp8, lse, n_first, beta, true, cuda_stream);
+    return attn_impl(Q, K, V, row_ptr, col_idx, false, scale, dtype, O, shape, fp8, lse, n_first, beta, true, cuda_stream);
+}
+
+chorus_status chorus_block_sparse_attn_fwd_idx16(const void* Q, const void* K, const void* V,
+                                                 const int32_t* row_ptr, const uint16_t* col_idx,
+                                                 float scale, chorus_dtype dtype, void* O,
+                                                 const chorus_attn_shape* shape,
+                                                 const chorus_fp8_scales* fp8, float* lse,
+                                                 int n_first, float beta, int geometry_64x128,
+                                                 void* cuda_stream) {
+    return attn_impl(Q, K, V, row_ptr, col_idx, true, scale, dtype, O, shape, fp8, lse, n_first, beta,
+                     geometry_64x128 != 0, cuda_stream);
 }
 
 static chorus_status attn_impl(const void* Q, const void* K, const void* V, const int32_t* row_ptr,
-                               const int32_t* col_idx, float scale, chorus_dtype dtype, void* O,
+                               const void* col_idx, bool idx16, float scale, chorus_dtype dtype, void* O,
                                const chorus_attn_shape* shape, const chorus_fp8_scales* fp8, float* lse,
                                int n_first, float beta, bool half_flags, void* cuda_stream) {
     g_err[0] = 0;
@@ -323,11 +369,14 @@ static chorus_status attn_impl(const void* Q, const void* K, const void* V, cons
     AttnParams p;
     p.row_ptr = row_ptr;
     p.col_idx = col_idx;
+    p.idx16 = idx16;
     p.O = O;
     p.o_sb = s.o_stride_b; p.o_sn = s.o_stride_n; p.o_sh = s.o_stride_h;
     p.B = s.B; p.H = s.H; p.N = s.N;
     p.nq = (s.N + CHORUS_BLOCK_Q - 1) / CHORUS_BLOCK_Q;
     p.nk = (s.N + CHORUS_BLOCK_K - 1) / CHORUS_BLOCK_K;
+    if (idx16 && p.nk > (half_flags ? 16384 : 65536))
+        return set_error(CHORUS_ERR_UNSUPPORTED, "%d key blocks do not fit the 16-bit index", p.nk);
     p.scale_log2 = scale * 1.4426950408889634f;
     p.q_scale = fp8 ? fp8->q_scale : nullptr;
     p.k_scale = fp8 ? fp8->k_scale : nullptr;

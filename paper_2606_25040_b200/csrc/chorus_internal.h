@@ -15,12 +15,13 @@ void count_launch(int n = 1);
 
 // ---- mask_decode.cu ----------------------------------------------------------------------------
 size_t decode_workspace_bytes(int64_t rows, int words);
+// col_idx: int32 entries, or uint16 entries when idx16
 cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, int words,
-                               int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
+                               int32_t* row_ptr, void* col_idx, bool idx16, int64_t col_cap, void* workspace,
                                cudaStream_t stream);
 size_t decode_64x128_workspace_bytes(int64_t heads, int N);
 cudaError_t launch_mask_decode_64x128(const uint32_t* bm64, int64_t heads, int N, int32_t* row_ptr,
-                                      int32_t* col_idx, int64_t col_cap, void* workspace, cudaStream_t stream);
+                                      void* col_idx, bool idx16, int64_t col_cap, void* workspace, cudaStream_t stream);
 cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_layer, int words,
                                  int nk, int group, cudaStream_t stream);
 
@@ -39,7 +40,8 @@ cudaError_t launch_quantize_fp8(const void* Q, const void* K, const void* V,
 // ---- attn_fwd.cu -------------------------------------------------------------------------------
 struct AttnParams {
     const int32_t* row_ptr;
-    const int32_t* col_idx;
+    const void* col_idx;   // int32 entries, or uint16 entries when idx16 (flags of the 64 x 128 form at bits 14 / 15)
+    bool idx16;
     void* O;
     int64_t o_sb, o_sn, o_sh;
     int B, H, N, nq, nk;

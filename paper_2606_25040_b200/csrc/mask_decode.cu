@@ -19,12 +19,9 @@
 namespace chorus {
 namespace {
 
-#ifndef CHORUS_DEC_STAGE
-#define CHORUS_DEC_STAGE 9216
-#endif
 constexpr int DEC_THREADS = 256;
 constexpr int DEC_WARPS = DEC_THREADS / 32;
-constexpr int STAGE = CHORUS_DEC_STAGE;                          // col_idx entries staged per round
+constexpr int STAGE = 9216;                                      // col_idx entries staged per round
 
 // per-tile status word: bits 63..62 = state (0 empty, 1 aggregate of the tile, 2 inclusive prefix),
 // low 32 bits = value.  Written and read with single 64-bit relaxed accesses.
@@ -76,12 +73,22 @@ __device__ __forceinline__ int32_t geo_entry(int t, int b, uint32_t fu, uint32_t
     return static_cast<int32_t>(static_cast<uint32_t>(t) | (nu << 30) | (nl << 31));
 }
 
+// A staged entry on its way out: 32-bit as it is; 16-bit with the two per-half flags of the
+// 64 x 128 geometry moved from bits 30 / 31 to bits 14 / 15.
+template <typename IdxT, bool kGeo>
+__device__ __forceinline__ IdxT out_entry(int32_t e) {
+    if constexpr (sizeof(IdxT) == 4) return static_cast<IdxT>(e);
+    const uint32_t u = static_cast<uint32_t>(e);
+    if constexpr (kGeo) return static_cast<IdxT>((u & 0x3fffu) | ((u >> 30) << 14));
+    return static_cast<IdxT>(u);
+}
+
 // WPT consecutive words per thread: 4 for large mask sets (fewer scans, divisions and status words per
 // word), 1 for a single layer (more, smaller tiles: one 480p layer is only 160 K words)
-template <int WPT, bool kGeo>
+template <int WPT, bool kGeo, typename IdxT>
 __global__ void __launch_bounds__(DEC_THREADS)
 decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, int words,
-                    int32_t* __restrict__ row_ptr, int32_t* __restrict__ col_idx, int64_t col_cap,
+                    int32_t* __restrict__ row_ptr, IdxT* __restrict__ col_idx, int64_t col_cap,
                     unsigned long long* __restrict__ status /* [0] = ticket counter, [1 + t] = tile t */,
                     const GeoSrc geo) {
     // entry e sits at e + e/32: threads whose runs start 8, 16 or 32 entries apart (25 %, 50 %, full
@@ -210,7 +217,7 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
     if (col_idx == nullptr) return;
     if (fast) {     // staged before the look-back; the __syncthreads after it ordered the writes
         for (int t = threadIdx.x; t < tile_total; t += DEC_THREADS)
-            if (base + t < col_cap) col_idx[base + t] = s_stage[t + (t >> 5)];
+            if (base + t < col_cap) col_idx[base + t] = out_entry<IdxT, kGeo>(s_stage[t + (t >> 5)]);
         return;
     }
     // 3b. a fuller tile (WPT > 1 only): WPT rounds of one word per thread, so that every thread walks
@@ -252,7 +259,7 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
             }
             __syncthreads();
             for (int t = threadIdx.x; t < hi - lo; t += DEC_THREADS)
-                if (base + lo + t < col_cap) col_idx[base + lo + t] = s_stage[t + (t >> 5)];
+                if (base + lo + t < col_cap) col_idx[base + lo + t] = out_entry<IdxT, kGeo>(s_stage[t + (t >> 5)]);
             __syncthreads();
         }
     }
@@ -291,8 +298,9 @@ size_t decode_workspace_bytes(int64_t rows, int words) {
     return static_cast<size_t>(n_tiles_for(rows, words) + 1) * sizeof(unsigned long long) + 8;
 }
 
+template <typename IdxT>
 static cudaError_t launch_decode(const uint32_t* bitmask, const GeoSrc* geo, int64_t rows, int nk, int words,
-                                 int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
+                                 int32_t* row_ptr, IdxT* col_idx, int64_t col_cap, void* workspace,
                                  cudaStream_t stream) {
     const int64_t nt = n_tiles_for(rows, words);
     auto* status = reinterpret_cast<unsigned long long*>((reinterpret_cast<uintptr_t>(workspace) + 7) & ~uintptr_t(7));
@@ -302,20 +310,22 @@ static cudaError_t launch_decode(const uint32_t* bitmask, const GeoSrc* geo, int
     const bool one = wpt_for(rows * words) == 1;
     const GeoSrc g = geo ? *geo : GeoSrc{nullptr, 0, 0, 0, 0};
     if (geo) {
-        if (one) decode_tiles_kernel<1, true><<<grid, DEC_THREADS, 0, stream>>>(nullptr, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
-        else decode_tiles_kernel<4, true><<<grid, DEC_THREADS, 0, stream>>>(nullptr, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+        if (one) decode_tiles_kernel<1, true, IdxT><<<grid, DEC_THREADS, 0, stream>>>(nullptr, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+        else decode_tiles_kernel<4, true, IdxT><<<grid, DEC_THREADS, 0, stream>>>(nullptr, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
     } else {
-        if (one) decode_tiles_kernel<1, false><<<grid, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
-        else decode_tiles_kernel<4, false><<<grid, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+        if (one) decode_tiles_kernel<1, false, IdxT><<<grid, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+        else decode_tiles_kernel<4, false, IdxT><<<grid, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
     }
     count_launch(1);
     return cudaGetLastError();
 }
 
 cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, int words,
-                               int32_t* row_ptr, int32_t* col_idx, int64_t col_cap, void* workspace,
+                               int32_t* row_ptr, void* col_idx, bool idx16, int64_t col_cap, void* workspace,
                                cudaStream_t stream) {
-    return launch_decode(bitmask, nullptr, rows, nk, words, row_ptr, col_idx, col_cap, workspace, stream);
+    if (idx16)
+        return launch_decode<uint16_t>(bitmask, nullptr, rows, nk, words, row_ptr, static_cast<uint16_t*>(col_idx), col_cap, workspace, stream);
+    return launch_decode<int32_t>(bitmask, nullptr, rows, nk, words, row_ptr, static_cast<int32_t*>(col_idx), col_cap, workspace, stream);
 }
 
 cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_layer, int words,
@@ -337,11 +347,14 @@ size_t decode_64x128_workspace_bytes(int64_t heads, int N) {
 
 // One launch: the decode kernel reads the 64 x 128 mask rows directly (GeoSrc) and writes the flagged entries.
 cudaError_t launch_mask_decode_64x128(const uint32_t* bm64, int64_t heads, int N, int32_t* row_ptr,
-                                      int32_t* col_idx, int64_t col_cap, void* workspace, cudaStream_t stream) {
+                                      void* col_idx, bool idx16, int64_t col_cap, void* workspace, cudaStream_t stream) {
     const int nq64 = (N + 63) / 64, nq128 = (N + 127) / 128, nk128 = nq128, nk64 = nq64;
     const GeoSrc geo{bm64, nq64, nq128, nk128, (nk128 + 31) / 32};
-    return launch_decode(nullptr, &geo, heads * nq128, nk64, (nk64 + 31) / 32, row_ptr, col_idx, col_cap,
-                         workspace, stream);
+    if (idx16)
+        return launch_decode<uint16_t>(nullptr, &geo, heads * nq128, nk64, (nk64 + 31) / 32, row_ptr,
+                                       static_cast<uint16_t*>(col_idx), col_cap, workspace, stream);
+    return launch_decode<int32_t>(nullptr, &geo, heads * nq128, nk64, (nk64 + 31) / 32, row_ptr,
+                                  static_cast<int32_t*>(col_idx), col_cap, workspace, stream);
 }
 
 }  // namespace chorus
