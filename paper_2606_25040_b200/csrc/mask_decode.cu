@@ -23,6 +23,25 @@ constexpr int DEC_THREADS = 256;
 constexpr int DEC_WARPS = DEC_THREADS / 32;
 constexpr int STAGE = 9216;                                      // col_idx entries staged per round
 
+// Staging-buffer slot of entry e: the low five bits are XORed with the next five, so that threads whose runs
+// start 8, 16 or 32 entries apart (25 %, 50 %, full density) hit different banks when they all write their
+// k-th entry, while 32 consecutive entries still fall into 32 different banks for the copy-out.
+__device__ __forceinline__ int slot(int e) { return e ^ ((e >> 5) & 31); }
+
+// The set bits of x, ascending, into the staging buffer from entry e on.  Walked from the top bit down into
+// descending slots: the position of the highest set bit is ONE instruction (FLO), where the lowest one costs a
+// bit reversal as well.  val(b) gives the entry of bit b.
+template <typename F>
+__device__ __forceinline__ void walk_word(uint32_t x, int e, int32_t* s_stage, F val) {
+    int pos = e + __popc(x) - 1;
+    while (x) {
+        const int b = 31 - __clz(x);
+        x ^= 1u << b;
+        s_stage[slot(pos)] = val(b);
+        --pos;
+    }
+}
+
 // per-tile status word: bits 63..62 = state (0 empty, 1 aggregate of the tile, 2 inclusive prefix),
 // low 32 bits = value.  Written and read with single 64-bit relaxed accesses.
 constexpr unsigned long long ST_AGG = 1ull << 62, ST_INC = 2ull << 62;
@@ -91,9 +110,7 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
                     int32_t* __restrict__ row_ptr, IdxT* __restrict__ col_idx, int64_t col_cap,
                     unsigned long long* __restrict__ status /* [0] = ticket counter, [1 + t] = tile t */,
                     const GeoSrc geo) {
-    // entry e sits at e + e/32: threads whose runs start 8, 16 or 32 entries apart (25 %, 50 %, full
-    // density) then hit different banks when they all write their k-th entry
-    __shared__ int32_t s_stage[STAGE + STAGE / 32];
+    __shared__ int32_t s_stage[STAGE];           // entry e at slot(e)
     __shared__ int s_warp[DEC_WARPS];
     __shared__ int2 s_look[DEC_WARPS];
     __shared__ int s_tile, s_base;
@@ -162,14 +179,14 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
             int e = off, wr = win0;
 #pragma unroll
             for (int i = 0; i < WPT; ++i) {
-                uint32_t x = v[i];
                 const int kb0 = wr * 32;
-                while (x) {
-                    const int b = __ffs(x) - 1;
-                    x &= x - 1;
-                    s_stage[e + (e >> 5)] = kGeo ? geo_entry(kb0 + b, b, fu[i], fl[i]) : kb0 + b;
-                    ++e;
+                if constexpr (kGeo) {
+                    const uint32_t gu = fu[i], gl = fl[i];
+                    walk_word(v[i], e, s_stage, [&](int b) { return geo_entry(kb0 + b, b, gu, gl); });
+                } else {
+                    walk_word(v[i], e, s_stage, [&](int b) { return kb0 + b; });
                 }
+                e += __popc(v[i]);
                 if (++wr == words) wr = 0;
             }
         }
@@ -216,8 +233,11 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
     }
     if (col_idx == nullptr) return;
     if (fast) {     // staged before the look-back; the __syncthreads after it ordered the writes
-        for (int t = threadIdx.x; t < tile_total; t += DEC_THREADS)
-            if (base + t < col_cap) col_idx[base + t] = out_entry<IdxT, kGeo>(s_stage[t + (t >> 5)]);
+        // entries beyond col_cap are never written: clamp once, then 32-bit indices only
+        const int n_out = static_cast<int>(min(static_cast<int64_t>(tile_total), max(col_cap - base, static_cast<int64_t>(0))));
+        IdxT* dst = col_idx + base;
+#pragma unroll 4
+        for (int t = threadIdx.x; t < n_out; t += DEC_THREADS) dst[t] = out_entry<IdxT, kGeo>(s_stage[slot(t)]);
         return;
     }
     // 3b. a fuller tile (WPT > 1 only): WPT rounds of one word per thread, so that every thread walks
@@ -226,9 +246,8 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
     // sits behind the largest round in the staging buffer.
     if constexpr (WPT > 1) {
         constexpr int ROUND_MAX = DEC_THREADS * 32;
-        static_assert(ROUND_MAX + ROUND_MAX / 32 + TILE_WORDS <= STAGE + STAGE / 32,
-                      "staging buffer too small for a round plus the offset table");
-        int* s_woff = s_stage + ROUND_MAX + ROUND_MAX / 32;
+        static_assert(ROUND_MAX + TILE_WORDS <= STAGE, "staging buffer too small for a round plus the offset table");
+        int* s_woff = s_stage + ROUND_MAX;
         {
             int o = off;
 #pragma unroll
@@ -249,17 +268,15 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
             uint32_t x = 0u, gu = 0u, gl = 0u;
             if (g < n_words) x = kGeo ? geo_word(geo, gr, wr, gu, gl) : __ldg(bitmask + g);
             if (wr == words - 1) x &= last_mask;
-            int e = s_woff[j] - lo;
+            const int e = s_woff[j] - lo;
             const int kb0 = wr * 32;
-            while (x) {
-                const int b = __ffs(x) - 1;
-                x &= x - 1;
-                s_stage[e + (e >> 5)] = kGeo ? geo_entry(kb0 + b, b, gu, gl) : kb0 + b;
-                ++e;
-            }
+            if constexpr (kGeo) walk_word(x, e, s_stage, [&](int b) { return geo_entry(kb0 + b, b, gu, gl); });
+            else walk_word(x, e, s_stage, [&](int b) { return kb0 + b; });
             __syncthreads();
-            for (int t = threadIdx.x; t < hi - lo; t += DEC_THREADS)
-                if (base + lo + t < col_cap) col_idx[base + lo + t] = out_entry<IdxT, kGeo>(s_stage[t + (t >> 5)]);
+            const int n_out = static_cast<int>(min(static_cast<int64_t>(hi - lo), max(col_cap - base - lo, static_cast<int64_t>(0))));
+            IdxT* dst = col_idx + base + lo;
+#pragma unroll 4
+            for (int t = threadIdx.x; t < n_out; t += DEC_THREADS) dst[t] = out_entry<IdxT, kGeo>(s_stage[slot(t)]);
             __syncthreads();
         }
     }
