@@ -23,7 +23,9 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(_build())
+        # CHORUS_ORACLE_SANITIZE=1: the ASan + UBSan build (the process must preload libasan; see
+        # tests/test_oracle_sanitizers.py)
+        _lib = C.CDLL(_build(sanitize=os.environ.get("CHORUS_ORACLE_SANITIZE") == "1"))
         _lib.oracle_mask_to_index.restype = C.c_int64
         _lib.oracle_mask_to_index_64x128.restype = C.c_int64
         _lib.oracle_mask_to_index_u16.restype = C.c_int64

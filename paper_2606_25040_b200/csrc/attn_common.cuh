@@ -29,6 +29,59 @@ __device__ __forceinline__ int ld_col(const AttnParams& p, int64_t i) {
     return p.half_flags ? static_cast<int>((e & 0x3fffu) | ((e >> 14) << 30)) : static_cast<int>(e);
 }
 
+// ---- dynamic item order ------------------------------------------------------------------------------------------
+// The CTAs of a launch draw their work items from one counter instead of taking every gridDim-th item: rows of
+// reused masks differ in length ("assigns a different sparsity level to each attention head"), and
+// with a fixed share per CTA the longest share sets the kernel time.  Items are still handed out in head-major
+// order, so the CTAs in flight keep working on one or two heads and their K / V stay in L2.
+// The counter is one of a few device words that reset themselves: the last CTA of a launch to finish zeroes its
+// slot, so no memset precedes the kernel.  The producer warp draws an index and passes it to the other roles of the
+// CTA through a small ring in shared memory.
+constexpr int ITEM_RING = 4, TICKET_SLOTS = 64;
+static __device__ unsigned int g_item_ticket[TICKET_SLOTS], g_item_done[TICKET_SLOTS];
+
+struct ItemRing {
+    uint32_t full, empty;      // shared-memory addresses of ITEM_RING mbarriers each
+    volatile int* slots;       // ITEM_RING indices
+};
+// producer warp, converged: the k-th item of this CTA (-1: none left), announced to the consumers
+__device__ __forceinline__ int item_draw(const ItemRing& r, uint32_t k, int n_items, int ticket_slot) {
+    const uint32_t s = k % ITEM_RING;
+    mbar_wait(r.empty + 8 * s, ((k / ITEM_RING) & 1) ^ 1);
+    int idx = 0;
+    if ((threadIdx.x & 31) == 0)
+        idx = k == 0 ? static_cast<int>(blockIdx.x)
+                     : static_cast<int>(gridDim.x + atomicAdd(&g_item_ticket[ticket_slot], 1u));
+    idx = __shfl_sync(0xffffffffu, idx, 0);
+    if (idx >= n_items) idx = -1;
+    if ((threadIdx.x & 31) == 0) {
+        r.slots[s] = idx;
+        mbar_arrive(r.full + 8 * s);
+    }
+    return idx;
+}
+// any other warp (all lanes): the k-th item of this CTA as the producer announced it
+__device__ __forceinline__ int item_take(const ItemRing& r, uint32_t k) {
+    const uint32_t s = k % ITEM_RING;
+    mbar_wait(r.full + 8 * s, (k / ITEM_RING) & 1);
+    const int idx = r.slots[s];
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(r.empty + 8 * s);
+    return idx;
+}
+// one thread per CTA, after everything else: the last CTA of the launch resets the slot
+__device__ __forceinline__ void item_ticket_release(int ticket_slot) {
+    if (atomicAdd(&g_item_done[ticket_slot], 1u) == gridDim.x - 1) {
+        g_item_ticket[ticket_slot] = 0u;
+        g_item_done[ticket_slot] = 0u;
+        __threadfence();
+    }
+}
+inline int next_ticket_slot() {
+    static unsigned int n = 0;      // launches are enqueued by one thread at a time per process in practice; a
+    return static_cast<int>(n++ % TICKET_SLOTS);   // collision needs 64 launches of one kernel in flight at once
+}
+
 struct Item {
     int b, h, qb, r0, nt, np;
 };

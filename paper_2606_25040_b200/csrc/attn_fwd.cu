@@ -53,14 +53,15 @@ struct Cfg {
     static constexpr uint32_t SO_OFF = SV_OFF + VSTAGES * TILE_BYTES;   // O staging: 2 slabs (bf16 out)
     static constexpr uint32_t XCH_OFF = SO_OFF + 32768;   // f32 [128] m_ref hand-off, [2][2][128] epilogue (m, l)
     static constexpr uint32_t BAR_OFF = XCH_OFF + 2560;
-    static constexpr uint32_t SMEM_BYTES = BAR_OFF + 256;
+    static constexpr uint32_t SMEM_BYTES = BAR_OFF + 384;
     // mbarrier slots (8 bytes each) from BAR_OFF
     static constexpr uint32_t B_Q_FULL = 0, B_Q_EMPTY = 1, B_K_FULL = 2, B_K_EMPTY = B_K_FULL + KSTAGES,
         B_V_FULL = B_K_EMPTY + KSTAGES, B_V_EMPTY = B_V_FULL + VSTAGES, B_S_FULL = B_V_EMPTY + VSTAGES,
         B_P_READY = B_S_FULL + SBUFS, B_PV_DONE = B_P_READY + SBUFS, B_ITEM_DONE = B_PV_DONE + SBUFS,
-        B_O_FREE = B_ITEM_DONE + 1, B_COUNT = B_O_FREE + 1;
+        B_O_FREE = B_ITEM_DONE + 1, B_IT_FULL = B_O_FREE + 1, B_IT_EMPTY = B_IT_FULL + ITEM_RING,
+        B_COUNT = B_IT_EMPTY + ITEM_RING;
     static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
-    static_assert(B_COUNT * 8 + 8 <= 256, "barrier area too small");
+    static_assert(B_COUNT * 8 + 8 + 4 * ITEM_RING <= 384, "barrier area too small");
     // P = exp2(x - m_ref) <= 2^8 under the lazy-rescale threshold of 2^8 (log2 units below)
     static constexpr float RESCALE_THRESHOLD = 8.0f;
     // P V steps per 64-key tile: 16 keys (8 TMEM columns of bf16 / fp16 pairs) per MMA
@@ -99,6 +100,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_items = p.B * p.H * p.nq;
+    const ItemRing ring{bar(C::B_IT_FULL), bar(C::B_IT_EMPTY),
+                        reinterpret_cast<volatile int*>(gbase + C::BAR_OFF + 8 * C::B_COUNT + 8)};
 
     if (threadIdx.x == 0) {
         mbar_init(bar(C::B_Q_FULL), 1);
@@ -112,6 +115,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
         mbar_init(bar(C::B_ITEM_DONE), 1);
         mbar_init(bar(C::B_O_FREE), 8);
+        for (int i = 0; i < ITEM_RING; ++i) { mbar_init(bar(C::B_IT_FULL + i), 1); mbar_init(bar(C::B_IT_EMPTY + i), 9); }   // MMA warp + 8 softmax warps
         fence_mbar_init();
     }
     if (warp == MMA_WARP) tmem_alloc(bars + 8 * C::B_COUNT, TM_COLS);
@@ -138,7 +142,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 tma_load_4d(dst + 16384, tm, b, 64, row0, h, bb);
             };
             uint32_t g = 0, icnt = 0;   // pairs and non-empty items issued so far
-            for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
+            for (uint32_t kit = 0;; ++kit) {
+                const int idx = item_draw(ring, kit, n_items, p.ticket_slot);
+                if (idx < 0) break;
                 const Item it = get_item_uniform(p, idx);
                 if (it.nt == 0) continue;   // empty rows touch no barrier
                 mbar_wait(bar(C::B_Q_EMPTY), (icnt & 1) ^ 1);
@@ -193,7 +199,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
             const uint64_t dV = smem_desc_sw128(sV, 16384, 1024);
             uint32_t g0 = 0, icnt = 0;      // pairs before this item, non-empty items so far
-            for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
+            for (uint32_t kit = 0;; ++kit) {
+                const int idx = item_take(ring, kit);
+                if (idx < 0) break;
                 const Item it = get_item_uniform(p, idx);
                 if (it.nt == 0) continue;
                 mbar_wait(bar(C::B_Q_FULL), icnt & 1);
@@ -267,7 +275,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         volatile float* xe = xch + 128;          // [2 parity][m, l][128] epilogue exchange
         uint32_t g0 = 0;                         // pairs of all previous items (S buffer / phase)
         uint32_t icnt = 0;                       // non-empty items so far
-        for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
+        for (uint32_t kit = 0;; ++kit) {
+            const int idx = item_take(ring, kit);
+            if (idx < 0) break;
             const Item it = get_item(p, idx);
             float m_ref = -INFINITY, l0 = 0.f, l1 = 0.f;
             // FP8 (R10): scores are (q8 . k8) * s_q[qb] * s_k[kb / 2]; the per-tile factor is
@@ -567,6 +577,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     tc_fence_before();
     __syncthreads();
     if (warp == MMA_WARP) tmem_dealloc(tmem, TM_COLS);
+    if (threadIdx.x == 0) item_ticket_release(p.ticket_slot);
 }
 
 }  // namespace
@@ -582,7 +593,9 @@ static cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, co
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     const int n_items = p.B * p.H * p.nq;
     const int grid = n_items < sms ? n_items : sms;
-    attn_fwd_kernel<kF16, kBeta, kHalf><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, p);
+    AttnParams pl = p;
+    pl.ticket_slot = next_ticket_slot();
+    attn_fwd_kernel<kF16, kBeta, kHalf><<<grid, NUM_THREADS, smem, stream>>>(tmQ, tmK, tmV, tmO, pl);
     count_launch(1);
     return cudaGetLastError();
 }

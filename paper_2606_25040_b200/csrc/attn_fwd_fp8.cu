@@ -41,14 +41,15 @@ constexpr uint32_t HALF = 8192;         // the second tile of a pair
 constexpr uint32_t SQ_OFF = 0, SK_OFF = TILE, SV_OFF = SK_OFF + KSTAGES * TILE, ONES_OFF = SV_OFF + VSTAGES * TILE,
                    ONES_BYTES = 4096,   // [32 keys][128 B] of e4m3 1.0: one K = 32 MMA step's worth
                    SO_OFF = ONES_OFF + ONES_BYTES, XCH_OFF = SO_OFF + 32768, BAR_OFF = XCH_OFF + 512,
-                   SMEM_BYTES = BAR_OFF + 256;
+                   SMEM_BYTES = BAR_OFF + 384;
 static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
 // mbarrier slots
 constexpr uint32_t B_Q_FULL = 0, B_Q_EMPTY = 1, B_K_FULL = 2, B_K_EMPTY = B_K_FULL + KSTAGES,
                    B_V_FULL = B_K_EMPTY + KSTAGES, B_V_EMPTY = B_V_FULL + VSTAGES, B_S_FULL = B_V_EMPTY + VSTAGES,
                    B_S_FREE = B_S_FULL + SBUFS, B_P_READY = B_S_FREE + SBUFS, B_PV_DONE = B_P_READY + PBUFS,
-                   B_ITEM_DONE = B_PV_DONE + PBUFS, B_O_FREE = B_ITEM_DONE + 1, B_COUNT = B_O_FREE + 1;
-static_assert(B_COUNT * 8 + 8 <= 256, "barrier area too small");
+                   B_ITEM_DONE = B_PV_DONE + PBUFS, B_O_FREE = B_ITEM_DONE + 1, B_IT_FULL = B_O_FREE + 1,
+                   B_IT_EMPTY = B_IT_FULL + ITEM_RING, B_COUNT = B_IT_EMPTY + ITEM_RING;
+static_assert(B_COUNT * 8 + 8 + 4 * ITEM_RING <= 384, "barrier area too small");
 // tensor-memory map (columns)
 constexpr uint32_t TM_O = 0, TM_L = 128, TM_S = 160, TM_P = 416, TM_COLS = 512;
 constexpr uint32_t PV_N = 144;          // 128 channels + 16 ones columns (M = 128 needs N % 16 == 0)
@@ -82,6 +83,7 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_items = p.B * p.H * p.nq;
+    const ItemRing ring{bar(B_IT_FULL), bar(B_IT_EMPTY), reinterpret_cast<volatile int*>(gbase + BAR_OFF + 8 * B_COUNT + 8)};
 
     if (threadIdx.x == 0) {
         mbar_init(bar(B_Q_FULL), 1);
@@ -92,6 +94,7 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
         for (int i = 0; i < PBUFS; ++i) { mbar_init(bar(B_P_READY + i), 4); mbar_init(bar(B_PV_DONE + i), 1); }
         mbar_init(bar(B_ITEM_DONE), 1);
         mbar_init(bar(B_O_FREE), 8);
+        for (int i = 0; i < ITEM_RING; ++i) { mbar_init(bar(B_IT_FULL + i), 1); mbar_init(bar(B_IT_EMPTY + i), 9); }   // MMA warp + 8 softmax warps
         fence_mbar_init();
     }
     // the ones slab: e4m3 1.0 = 0x38 in every byte (constant, so the 128-byte swizzle does not matter)
@@ -114,7 +117,9 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
         // everything an issue needs is made warp-uniform first (see attn_fwd.cu).
         if (warp == PRODUCER_WARP) {
             uint32_t g = 0, icnt = 0;   // pairs and non-empty items issued so far
-            for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
+            for (uint32_t kit = 0;; ++kit) {
+                const int idx = item_draw(ring, kit, n_items, p.ticket_slot);
+                if (idx < 0) break;
                 const Item it = get_item_uniform(p, idx);
                 if (it.nt == 0) continue;   // empty rows touch no barrier
                 mbar_wait(bar(B_Q_EMPTY), (icnt & 1) ^ 1);
@@ -168,7 +173,9 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
             const uint64_t dQ = smem_desc_sw128(sQ, 16, 1024);
             const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
             uint32_t g0 = 0, icnt = 0;      // pairs before this item, non-empty items so far
-            for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
+            for (uint32_t kit = 0;; ++kit) {
+                const int idx = item_take(ring, kit);
+                if (idx < 0) break;
                 const Item it = get_item_uniform(p, idx);
                 if (it.nt == 0) continue;
                 mbar_wait(bar(B_Q_FULL), icnt & 1);
@@ -234,7 +241,9 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
         const int nsb = (p.N + 127) >> 7;        // Q/K scale blocks of 128 tokens
         uint32_t g0 = 0;                         // pairs of all previous items
         uint32_t icnt = 0;                       // non-empty items so far
-        for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
+        for (uint32_t kit = 0;; ++kit) {
+            const int idx = item_take(ring, kit);
+            if (idx < 0) break;
             const Item it = get_item(p, idx);
             float m_ref = -INFINITY;
             // scores are (q8 . k8) * s_q[qb] * s_k[kb / 2] (R10); the per-tile factor is folded into the
@@ -453,6 +462,7 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
     tc_fence_before();
     __syncthreads();
     if (warp == MMA_WARP) tmem_dealloc(tmem, TM_COLS);
+    if (threadIdx.x == 0) item_ticket_release(p.ticket_slot);
 }
 
 template <bool kBeta, bool kHalf>
@@ -465,7 +475,9 @@ cudaError_t launch_one(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUt
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     const int n_items = p.B * p.H * p.nq;
     const int grid = n_items < sms ? n_items : sms;
-    attn_fwd_fp8_kernel<kBeta, kHalf><<<grid, NUM_THREADS, SMEM_BYTES, stream>>>(tmQ, tmK, tmV, tmO, p);
+    AttnParams pl = p;
+    pl.ticket_slot = next_ticket_slot();
+    attn_fwd_fp8_kernel<kBeta, kHalf><<<grid, NUM_THREADS, SMEM_BYTES, stream>>>(tmQ, tmK, tmV, tmO, pl);
     count_launch(1);
     return cudaGetLastError();
 }

@@ -53,6 +53,7 @@ struct AttnParams {
     int n_first;  // first-frame key enhancement (eq. 1): scores of keys < n_first are multiplied by beta
     float beta;   // > 0; n_first = 0 or beta = 1 selects the plain kernel
     bool half_flags;  // col_idx entries carry bits 30 / 31 (chorus_mask_to_index_64x128)
+    int ticket_slot;  // which self-resetting work counter this launch draws its items from (set by the launcher)
 };
 cudaError_t launch_attn_fwd(const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
                             const CUtensorMap& tmO, const AttnParams& p, chorus_dtype dtype,
