@@ -718,6 +718,21 @@ def run_chorus(args):
                 ts.append(a.elapsed_time(b_))
         set_ms = statistics.median(ts)
         set_bytes = 4 * rows_s * cfg.words + 4 * (rows_s + 1) + 4 * int(rp_s[-1].item())
+        # the same set with 16-bit entries (chorus_mask_to_index_u16: half the dominant write)
+        ci_s16 = torch.empty(ci_s.numel(), dtype=torch.uint16, device=dev)
+        ts = []
+        for i in range(8):
+            flush.zero_()
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            B.chorus_mask_to_index(dMs, cfg.nk, row_ptr=rp_s, col_idx=ci_s16, workspace=ws_s)
+            b_.record(stream)
+            torch.cuda.synchronize()
+            if i >= 3:
+                ts.append(a.elapsed_time(b_))
+        set16_ms = statistics.median(ts)
+        set16_bytes = 4 * rows_s * cfg.words + 4 * (rows_s + 1) + 2 * int(rp_s[-1].item())
+        del ci_s16
         # one layer alone with a cold L2 (the step's own decode_ms follows an attention kernel, warm)
         ts = []
         for i in range(8):
@@ -783,7 +798,9 @@ def run_chorus(args):
                                   "decode_set_GBps": set_bytes / (set_ms * 1e-3) / 1e9,
                                   "decode_set_frac_of_hbm": set_bytes / (set_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                                   "decode_set": "40 layers x %d heads x %d rows, L2 flushed, median of 5" % (cfg.H, cfg.nq),
-                                  "decode_layer_cold_l2_ms": layer_cold_ms})
+                                  "decode_layer_cold_l2_ms": layer_cold_ms,
+                                  "decode_set_u16_ms": set16_ms, "decode_set_u16_bytes": set16_bytes,
+                                  "decode_set_u16_frac_of_hbm": set16_bytes / (set16_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]})
     if has_fp8:
         a8 = my_flops / (attn8_ms * 1e-3) / 1e12
         line["breakdown"].update({"quantize_ms": quant_ms, "attn_fp8_ms": attn8_ms, "attn_fp8_TFLOPs": a8,
