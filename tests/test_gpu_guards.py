@@ -1,6 +1,6 @@
 """Out-of-bounds guards: every output buffer sits between sentinel regions, and after each call the
-sentinels must be intact (compute-sanitizer is not available on the GPU pool, so the tests carry their
-own bounds checks).  Ragged shapes on purpose: N = 3120 has a 48-row last query block / 48-key last
+sentinels must be intact (compute-sanitizer is closed on the GPU pool - its exact answer is quoted in DESIGN.md
+section 7.5 - so the tests carry their own bounds checks).  Ragged shapes on purpose: N = 3120 has a 48-row last query block / 48-key last
 key block."""
 import numpy as np
 import pytest
