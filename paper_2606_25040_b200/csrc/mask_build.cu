@@ -19,22 +19,28 @@ using namespace ptx;
 // =================================================================================================
 // block mass
 // =================================================================================================
-// Persistent kernel, one CTA (384 threads) per SM, work item = one (batch, head, 128-row query
-// block).  Keys are taken 128 at a time ("a pair" of 64-key blocks); an item makes 2 * P steps
-// over its P pairs: steps 0..P-1 give every row its running maximum and sum (-> log-sum-exp), steps
-// P..2P-1 recompute the same scores and sum exp2(s - lse) over the rows and the 64 columns of each
-// block.  Recomputing QK^T costs a second MMA pass, but nothing of size N x N is ever stored.
-// When the caller hands in the rows' log-sum-exp (an output of the dense attention call that the
-// historical request makes anyway), the first pass is skipped (template kLse).
-//   warp 8      TMA producer: Q once per item, then the K pair of every step (ring of KST stages)
-//   warp 9      MMA issuer: S = Q K^T (M=128, N=128, K=128, bf16 -> fp32) into one of four S buffers
-//               in tensor memory, up to four steps ahead of the readers
-//   warps 0-3   read the even steps, warps 4-7 the odd ones; warp w owns TMEM lanes 32*(w%4)..
-//               (one query row per thread); an S buffer is released as soon as it is in registers
-constexpr int MB_THREADS = 384, MB_PRODUCER = 8, MB_MMA = 9;
-constexpr int KST = 5, SB = 4;
+// Persistent kernel, one CTA (576 threads) per SM, work item = one (batch, head, 256-row query
+// block): TWO 128-row query tiles share every key tile that is brought in.  Keys are taken 128 at a
+// time ("a pair" of 64-key blocks); an item makes 2 * P steps over its P pairs: steps 0..P-1 give
+// every row its running maximum and sum (-> log-sum-exp), steps P..2P-1 recompute the same scores and
+// sum exp2(s - lse) over the rows and the 64 columns of each block.  Recomputing QK^T costs a second
+// MMA pass, but nothing of size N x N is ever stored.  When the caller hands in the rows' log-sum-exp
+// (an output of the dense attention call that the historical request makes anyway), the
+// first pass is skipped (template kLse).
+//   warp 16     TMA producer: the two Q tiles once per item, then the K pair of every step (ring of KST stages)
+//   warp 17     MMA issuer: per step S_q = Q_q K^T (M=128, N=128, K=128, bf16 -> fp32) for q = 0, 1 into
+//               two of four S buffers in tensor memory, one step ahead of the readers
+//   warps 0-15  four groups of four: group (q, parity) reads query tile q on the steps of that parity, i.e.
+//               it owns S buffer 2 * parity + q; warp w owns TMEM lanes 32*(w%4).. (one query row per
+//               thread); an S buffer is released as soon as it is in registers.  Four reader warps per
+//               scheduler (at <= 112 registers) keep its MUFU busy: one warp's exponential pass is paced
+//               by ptxas at one MUFU.EX2 per 8 cycles, the pipe's own rate, and every stall of a lone warp
+//               is a stall of the pipe (80 % MUFU utilisation with four warps, 54 % with two).
+constexpr int MB_THREADS = 576, MB_READERS = 16, MB_PRODUCER = 16, MB_MMA = 17;
+constexpr int KST = 4, SB = 4;
+constexpr uint32_t MASS_POLY = 0x49u;                  // element pairs 0, 3, 6 of every 8: polynomial exp2
 constexpr uint32_t TILE = 32768;                       // 128 rows x 128 bf16 channels (two slabs)
-constexpr uint32_t M_SQ = 0, M_SK = TILE, M_XCH = M_SK + KST * TILE, M_BAR = M_XCH + 4096,
+constexpr uint32_t M_SQ = 0, M_SK = 2 * TILE, M_XCH = M_SK + KST * TILE, M_BAR = M_XCH + 4096 + 512,
                    M_SMEM = M_BAR + 256;
 // mbarrier slots
 constexpr uint32_t B_Q_FULL = 0, B_Q_EMPTY = 1, B_K_FULL = 2, B_K_EMPTY = B_K_FULL + KST,
@@ -59,11 +65,12 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const uint32_t sQ = base + M_SQ, sK = base + M_SK, bars = base + M_BAR;
     auto bar = [&](uint32_t i) { return bars + 8u * i; };
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem_raw + M_BAR + 8 * B_CNT);
-    volatile float* xst = reinterpret_cast<volatile float*>(smem_raw + M_XCH);          // [2 groups][m, l][128]
-    volatile float* xpart = reinterpret_cast<volatile float*>(smem_raw + M_XCH + 2048); // [2 groups][2 bufs][4 warps][2]
+    volatile float* xst = reinterpret_cast<volatile float*>(smem_raw + M_XCH);            // [2 tiles][2 parities][m, l][128]
+    volatile float* xpart = reinterpret_cast<volatile float*>(smem_raw + M_XCH + 4096);   // [4 groups][2 bufs][4 warps][2]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_items = p.B * p.H * p.nq;
+    const int nq2 = (p.nq + 1) >> 1;     // 256-row items per head
+    const int n_items = p.B * p.H * nq2;
     const int P = (p.nk + 1) >> 1;       // pairs per item
     // With the rows' log-sum-exp given (an output of the dense attention call) the first pass is
     // skipped: P steps instead of 2 P, one exponential per score instead of two.
@@ -85,12 +92,15 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     if (warp == MB_PRODUCER) {
         uint32_t st = 0, ph = 0, icnt = 0;
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x, ++icnt) {
-            const int qb = idx % p.nq, bh = idx / p.nq, h = bh % p.H, b = bh / p.H;
+            const int qb2 = idx % nq2, bh = idx / nq2, h = bh % p.H, b = bh / p.H;
             mbar_wait(bar(B_Q_EMPTY), (icnt & 1) ^ 1);
             if (elect_one()) {
-                mbar_arrive_expect_tx(bar(B_Q_FULL), TILE);
-                tma_load_4d(sQ, &tmQ, bar(B_Q_FULL), 0, qb * 128, h, b);
-                tma_load_4d(sQ + 16384, &tmQ, bar(B_Q_FULL), 64, qb * 128, h, b);
+                // rows >= N (the second tile of an odd last item included) arrive as zeros
+                mbar_arrive_expect_tx(bar(B_Q_FULL), 2 * TILE);
+                for (int q = 0; q < 2; ++q) {
+                    tma_load_4d(sQ + q * TILE, &tmQ, bar(B_Q_FULL), 0, (2 * qb2 + q) * 128, h, b);
+                    tma_load_4d(sQ + q * TILE + 16384, &tmQ, bar(B_Q_FULL), 64, (2 * qb2 + q) * 128, h, b);
+                }
             }
             __syncwarp();
             for (int t = 0; t < T; ++t) {
@@ -110,63 +120,108 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         constexpr uint32_t IDESC = make_idesc(1u, 1u, 128, 128, 0, 0);    // bf16 x bf16 -> fp32
         const uint64_t dQ = smem_desc_sw128(sQ, 16, 1024);
         const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
-        uint32_t st = 0, ph = 0, icnt = 0, g = 0;
+        uint32_t st = 0, ph = 0, icnt = 0, g = 0;      // g: steps so far; step g writes S buffers 2 (g & 1) + q
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x, ++icnt) {
             mbar_wait(bar(B_Q_FULL), icnt & 1);
             for (int t = 0; t < T; ++t, ++g) {
-                const uint32_t sb = g % SB;
                 mbar_wait(bar(B_K_FULL + st), ph);
-                if (g >= SB) mbar_wait(bar(B_S_FREE + sb), ((g - SB) / SB) & 1);
-                tc_fence_after();
-                if (elect_one()) {
-                    const uint32_t tS = tmem + sb * 128;
-                    const uint64_t dKs = dK + ((st * TILE) >> 4);
+                for (int q = 0; q < 2; ++q) {
+                    const uint32_t sb = 2 * (g & 1) + q;
+                    if (g >= 2) mbar_wait(bar(B_S_FREE + sb), ((g >> 1) - 1) & 1);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint32_t tS = tmem + sb * 128;
+                        const uint64_t dQq = dQ + ((q * TILE) >> 4);
+                        const uint64_t dKs = dK + ((st * TILE) >> 4);
 #pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) {     // 16 bf16 channels = 32 B per step, 2 slabs
-                        const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
-                        mma_f16_ss(tS, dQ + off, dKs + off, IDESC, ks > 0);
+                        for (int ks = 0; ks < 8; ++ks) {     // 16 bf16 channels = 32 B per step, 2 slabs
+                            const uint32_t off = ((ks >> 2) * 16384 + (ks & 3) * 32) >> 4;
+                            mma_f16_ss(tS, dQq + off, dKs + off, IDESC, ks > 0);
+                        }
+                        tc_commit(bar(B_S_FULL + sb));
+                        if (q == 1) {
+                            tc_commit(bar(B_K_EMPTY + st));
+                            if (t == T - 1) tc_commit(bar(B_Q_EMPTY));
+                        }
                     }
-                    tc_commit(bar(B_K_EMPTY + st));
-                    tc_commit(bar(B_S_FULL + sb));
-                    if (t == T - 1) tc_commit(bar(B_Q_EMPTY));
+                    __syncwarp();
                 }
-                __syncwarp();
                 if (++st == KST) { st = 0; ph ^= 1; }
             }
         }
-    } else if (warp < 8) {
-        const int grp = warp >> 2, wq = warp & 3, row = wq * 32 + lane;
+    } else if (warp < MB_READERS) {
+        // group = (query tile of the item, parity of the steps it reads): it owns S buffer 2 * parity + tile
+        const int grp = warp >> 2, tile = grp & 1, par = grp >> 1, wq = warp & 3, row = wq * 32 + lane;
         const uint32_t tlane = tmem + (static_cast<uint32_t>(wq * 32) << 16);
         const float sl2 = p.scale_log2;
         uint32_t g0 = 0;                        // steps of all previous items
+        uint32_t own = 0;                       // mass steps of this group so far (xpart buffer)
         for (int idx = blockIdx.x; idx < n_items; idx += gridDim.x) {
-            const int qb = idx % p.nq;
+            const int qb = 2 * (idx % nq2) + tile;          // this group's 128-row query block
+            const int64_t bh = idx / nq2;
+            const bool tile_ok = qb < p.nq;                 // the second tile of an odd last item does not exist
             const bool row_ok = qb * 128 + row < p.N;
             float m = -INFINITY, l = 0.f, lse2 = 0.f;
             if (kLse && row_ok)                 // natural log -> the log2 domain of the scores
-                lse2 = __ldg(p.lse + static_cast<int64_t>(idx / p.nq) * p.N + qb * 128 + row) * 1.4426950408889634f;
-            uint32_t own = 0;                   // this group's steps of the item so far (xpart buffer)
+                lse2 = __ldg(p.lse + bh * p.N + qb * 128 + row) * 1.4426950408889634f;
             for (int t = 0; t < T; ++t) {
                 if (!kLse && t == P) {
-                    // ---- pass boundary: combine the two groups' (m, l) into the row's log-sum-exp
-                    xst[(grp * 2 + 0) * 128 + row] = m;
-                    xst[(grp * 2 + 1) * 128 + row] = l;
-                    named_bar_sync(1, 256);
-                    const float mo = xst[((grp ^ 1) * 2 + 0) * 128 + row], lo = xst[((grp ^ 1) * 2 + 1) * 128 + row];
+                    // ---- pass boundary: the two groups of a tile combine their (m, l) into the row's log-sum-exp
+                    xst[((tile * 2 + par) * 2 + 0) * 128 + row] = m;
+                    xst[((tile * 2 + par) * 2 + 1) * 128 + row] = l;
+                    named_bar_sync(6 + tile, 256);
+                    const float mo = xst[((tile * 2 + (par ^ 1)) * 2 + 0) * 128 + row];
+                    const float lo = xst[((tile * 2 + (par ^ 1)) * 2 + 1) * 128 + row];
                     const float M = fmaxf(m, mo);           // finite: every row sees at least one key
                     const float L = (m == -INFINITY ? 0.f : l * ex2(m - M)) + (mo == -INFINITY ? 0.f : lo * ex2(mo - M));
                     lse2 = M + lg2(L);
-                    named_bar_sync(1, 256);                  // both have read: the slots may be rewritten
+                    named_bar_sync(6 + tile, 256);           // both have read: the slots may be rewritten
                 }
                 const uint32_t g = g0 + t;
-                if ((g & 1) != static_cast<uint32_t>(grp)) continue;
-                const uint32_t sb = g % SB;
+                if ((g & 1) != static_cast<uint32_t>(par)) continue;
+                const uint32_t sb = 2 * par + tile;
                 const int j = t < P ? t : t - P;
                 const int valid = min(128, p.N - j * 128);   // keys of this pair that exist
-                mbar_wait(bar(B_S_FULL + sb), (g / SB) & 1);
+                mbar_wait(bar(B_S_FULL + sb), (g >> 1) & 1);
                 tc_fence_after();
                 const uint32_t tS = tlane + sb * 128;
                 float sum_a = 0.f, sum_b = 0.f;
+                if ((kLse || t >= P) && valid == 128) {
+                    // ---- the common step (mass pass, all 128 keys exist): the four 32-column chunks are streamed
+                    // with the next chunk's load in flight, packed FFMA2 / FADD2, and three of every 8 element
+                    // pairs (MASS_POLY) take their exponential from the degree-3 polynomial on the FMA pipe
+                    // (relative error 1e-4; tolerance of the masses 2e-3)
+                    const float2 sl2_2 = make_float2(sl2, sl2), nlse_2 = make_float2(-lse2, -lse2);
+                    auto chunk = [&](const uint32_t (&r)[32], float2& acc) {
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) {
+                            const float2 x = ffma2(make_float2(__uint_as_float(r[2 * q]), __uint_as_float(r[2 * q + 1])),
+                                                   sl2_2, nlse_2);
+                            const float2 e = ((MASS_POLY >> (q & 7)) & 1u) ? exp2_poly2<3>(x)
+                                                                           : make_float2(ex2(x.x), ex2(x.y));
+                            acc = fadd2(acc, e);
+                        }
+                    };
+                    uint32_t ra[32], rb[32];
+                    float2 acc_a = make_float2(0.f, 0.f), acc_b = make_float2(0.f, 0.f);
+                    tmem_ld32(tS, ra);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 32, rb);
+                    chunk(ra, acc_a);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 64, ra);
+                    chunk(rb, acc_a);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 96, rb);
+                    chunk(ra, acc_b);
+                    tc_wait_ld();
+                    tc_fence_before();                       // the buffer is in registers: hand it back
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(B_S_FREE + sb));
+                    chunk(rb, acc_b);
+                    sum_a = acc_a.x + acc_a.y;
+                    sum_b = acc_b.x + acc_b.y;
+                } else
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     uint32_t r[32];
@@ -212,21 +267,19 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     volatile float* part = xpart + ((grp * 2 + (own & 1)) * 4) * 2;
                     if (lane == 0) { part[wq * 2] = sum_a; part[wq * 2 + 1] = sum_b; }
                     named_bar_sync(2 + grp, 128);
-                    if (wq == 0 && lane == 0) {
+                    if (wq == 0 && lane == 0 && tile_ok) {
                         const float a = ((part[0] + part[2]) + part[4]) + part[6];
                         const float bsum = ((part[1] + part[3]) + part[5]) + part[7];
                         if (p.geo64) {
                             // 64 x 128 geometry: step j is key block j; warps 0-1 / 2-3 hold rows 0-63 / 64-127
                             const int nq64 = (p.N + 63) >> 6, nk128 = p.nq;
-                            const int qb = idx % p.nq;
-                            const int64_t bh = idx / p.nq;
                             float* out = p.mass + (bh * nq64 + 2 * qb) * nk128 + j;
                             out[0] = (part[0] + part[2]) + (part[1] + part[3]);
                             if (2 * qb + 1 < nq64) out[nk128] = (part[4] + part[6]) + (part[5] + part[7]);
                         } else {
-                        float* out = p.mass + static_cast<int64_t>(idx) * p.nk + 2 * j;
-                        out[0] = a;
-                        if (2 * j + 1 < p.nk) out[1] = bsum;
+                            float* out = p.mass + (bh * p.nq + qb) * p.nk + 2 * j;
+                            out[0] = a;
+                            if (2 * j + 1 < p.nk) out[1] = bsum;
                         }
                     }
                     ++own;
@@ -382,7 +435,7 @@ cudaError_t launch_block_mass(const CUtensorMap& tmQ, const CUtensorMap& tmK, co
     p.nk = (N + 63) / 64;
     p.scale_log2 = scale_log2;
     p.geo64 = geo64 ? 1 : 0;
-    const int n_items = B * H * p.nq;
+    const int n_items = B * H * ((p.nq + 1) / 2);
     const int grid = n_items < sms ? n_items : sms;
     if (lse) block_mass_kernel<true><<<grid, MB_THREADS, M_SMEM, stream>>>(tmQ, tmK, p);
     else block_mass_kernel<false><<<grid, MB_THREADS, M_SMEM, stream>>>(tmQ, tmK, p);
