@@ -35,7 +35,8 @@ template <typename F>
 __device__ __forceinline__ void walk_word(uint32_t x, int e, int32_t* s_stage, F val) {
     int pos = e + __popc(x) - 1;
     while (x) {
-        const int b = 31 - __clz(x);
+        int b;
+        asm("bfind.u32 %0, %1;" : "=r"(b) : "r"(x));   // one FLO; `31 - __clz(x)` compiles to a clz and its way back
         x ^= 1u << b;
         s_stage[slot(pos)] = val(b);
         --pos;
