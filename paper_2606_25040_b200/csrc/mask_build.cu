@@ -221,6 +221,48 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     chunk(rb, acc_b);
                     sum_a = acc_a.x + acc_a.y;
                     sum_b = acc_b.x + acc_b.y;
+                } else if (!kLse && t < P && valid == 128) {
+                    // ---- the common step of the first pass: online maximum and sum per 32-column chunk, streamed
+                    // and packed like the mass pass
+                    const float2 sl2_2 = make_float2(sl2, sl2);
+                    auto chunk1 = [&](const uint32_t (&r)[32]) {
+                        float a0 = -INFINITY, a1 = -INFINITY;
+#pragma unroll
+                        for (int k = 0; k < 32; k += 4) {
+                            a0 = fmaxf(fmaxf(a0, __uint_as_float(r[k])), __uint_as_float(r[k + 1]));
+                            a1 = fmaxf(fmaxf(a1, __uint_as_float(r[k + 2])), __uint_as_float(r[k + 3]));
+                        }
+                        const float mn = fmaxf(m, fmaxf(a0, a1) * sl2);      // sl2 > 0
+                        l *= ex2(m - mn);                                    // m = -inf: l is 0 and stays 0
+                        m = mn;
+                        const float2 nm_2 = make_float2(-m, -m);
+                        float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) {
+                            const float2 x = ffma2(make_float2(__uint_as_float(r[2 * q]), __uint_as_float(r[2 * q + 1])),
+                                                   sl2_2, nm_2);
+                            const float2 e = ((MASS_POLY >> (q & 7)) & 1u) ? exp2_poly2<3>(x)
+                                                                           : make_float2(ex2(x.x), ex2(x.y));
+                            acc = fadd2(acc, e);
+                        }
+                        l += acc.x + acc.y;
+                    };
+                    uint32_t ra[32], rb[32];
+                    tmem_ld32(tS, ra);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 32, rb);
+                    chunk1(ra);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 64, ra);
+                    chunk1(rb);
+                    tc_wait_ld();
+                    tmem_ld32(tS + 96, rb);
+                    chunk1(ra);
+                    tc_wait_ld();
+                    tc_fence_before();                       // the buffer is in registers: hand it back
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(B_S_FREE + sb));
+                    chunk1(rb);
                 } else
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
