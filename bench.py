@@ -440,6 +440,9 @@ def extras_block(cfg, dev, stream, dQ, dK, dV, dO, q8, dO8, rp, ci, peaks):
                          "roofline": {"kernel": "block_mass (one sweep)", "bound": "alu", "unit": "Gexp/s",
                                       "achieved": exps / (t1 * 1e-3) / 1e9, "peak": peak / 1e9,
                                       "frac": exps / (t1 * 1e-3) / peak,
+                                      "on_mufu": 0.625, "frac_mufu_only": 0.625 * exps / (t1 * 1e-3) / peak,
+                                      "note": "all N^2 H exponentials against the MUFU rate; 3 of 8 take the "
+                                              "degree-3 polynomial on the FMA pipe (frac_mufu_only counts 5 of 8)",
                                       "peak_source": "148 SMs x 16 MUFU lanes x max SM clock (DESIGN.md 6.6)"},
                          "mask_from_mass_ms": t_sel, "mask_coverage_ms": t_cov,
                          "kept_blocks_mean": float(kept.float().mean()), "coverage_mean": float(cov.mean())}
