@@ -164,21 +164,24 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             float m = -INFINITY, l = 0.f, lse2 = 0.f;
             if (kLse && row_ok)                 // natural log -> the log2 domain of the scores
                 lse2 = __ldg(p.lse + bh * p.N + qb * 128 + row) * 1.4426950408889634f;
-            for (int t = 0; t < T; ++t) {
-                if (!kLse && t == P) {
-                    // ---- pass boundary: the two groups of a tile combine their (m, l) into the row's log-sum-exp
-                    xst[((tile * 2 + par) * 2 + 0) * 128 + row] = m;
-                    xst[((tile * 2 + par) * 2 + 1) * 128 + row] = l;
-                    named_bar_sync(6 + tile, 256);
-                    const float mo = xst[((tile * 2 + (par ^ 1)) * 2 + 0) * 128 + row];
-                    const float lo = xst[((tile * 2 + (par ^ 1)) * 2 + 1) * 128 + row];
-                    const float M = fmaxf(m, mo);           // finite: every row sees at least one key
-                    const float L = (m == -INFINITY ? 0.f : l * ex2(m - M)) + (mo == -INFINITY ? 0.f : lo * ex2(mo - M));
-                    lse2 = M + lg2(L);
-                    named_bar_sync(6 + tile, 256);           // both have read: the slots may be rewritten
-                }
+            bool second = kLse;                  // the mass pass has begun (with an LSE given: from the start)
+            // pass boundary: the two groups of a tile combine their (m, l) into the row's log-sum-exp
+            auto boundary = [&]() {
+                second = true;
+                xst[((tile * 2 + par) * 2 + 0) * 128 + row] = m;
+                xst[((tile * 2 + par) * 2 + 1) * 128 + row] = l;
+                named_bar_sync(6 + tile, 256);
+                const float mo = xst[((tile * 2 + (par ^ 1)) * 2 + 0) * 128 + row];
+                const float lo = xst[((tile * 2 + (par ^ 1)) * 2 + 1) * 128 + row];
+                const float M = fmaxf(m, mo);               // finite: every row sees at least one key
+                const float L = (m == -INFINITY ? 0.f : l * ex2(m - M)) + (mo == -INFINITY ? 0.f : lo * ex2(mo - M));
+                lse2 = M + lg2(L);
+                named_bar_sync(6 + tile, 256);               // both have read: the slots may be rewritten
+            };
+            // this group's steps: those whose number g0 + t has its parity
+            for (int t = (par ^ static_cast<int>(g0 & 1u)); t < T; t += 2) {
+                if (!second && t >= P) boundary();
                 const uint32_t g = g0 + t;
-                if ((g & 1) != static_cast<uint32_t>(par)) continue;
                 const uint32_t sb = 2 * par + tile;
                 const int j = t < P ? t : t - P;
                 const int valid = min(128, p.N - j * 128);   // keys of this pair that exist
@@ -327,6 +330,7 @@ block_mass_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     ++own;
                 }
             }
+            if (!second) boundary();             // (a single pair: this group had no step in the mass pass)
             g0 += T;
         }
     }
