@@ -86,6 +86,28 @@ chorus_status chorus_mask_to_index(const uint32_t* bitmask, int L, int H, int nq
                                    void* workspace, size_t* workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * chorus_mask_to_index_static: chorus_mask_to_index (same operation; same bitmask,
+ * row_ptr, col_idx, col_cap and result, bit for bit) for callers that cannot allocate or hand in a
+ * workspace: code under CUDA graph capture, serving loops and harnesses that forbid cudaMalloc.
+ * The call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine): the kernel's
+ * scratch - one 8-byte status word per tile of the mask - is a file-scope device array of
+ * CHORUS_STATIC_DECODE_MAX_TILES + 1 words (128 KB), which every GPU that loads the library holds until
+ * exit.  Limit: the mask set may have at most CHORUS_STATIC_DECODE_MAX_WORDS = 2^24 32-bit words
+ * (L*H*nq_blk*ceil(nk_blk/32); 64 MiB of bitmask: 2.5 mask sets of 40 layers x 40 heads at 480p);
+ * larger sets are rejected with CHORUS_ERR_CAPACITY and nothing is launched.
+ * All calls on a device share the array: calls that overlap on the GPU (different streams, or
+ * different threads without ordering) RACE; calls ordered on one stream are fine.  The array keeps the
+ * previous call's contents; each call clears the words it uses on its own stream first.
+ * Errors: INVALID_ARG (null bitmask/row_ptr, sizes <= 0, col_cap < 0, misaligned pointers),
+ *         CAPACITY (L*H*nq_blk*nk_blk > INT32_MAX, or more words than the limit), CUDA.
+ * ------------------------------------------------------------------------------------------- */
+#define CHORUS_STATIC_DECODE_MAX_TILES 16384
+#define CHORUS_STATIC_DECODE_MAX_WORDS (1 << 24)
+chorus_status chorus_mask_to_index_static(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                          int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
+                                          void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Block-pair visit refreshing (PAPER.md:L93 (1); layer_flash = 8 at L153).  Within each group of
  * `group` consecutive layers a visited map V[h,q,k] records the block pairs activated so far;
  * "when executing the last layer of the group, any block pair that is still unvisited is forced

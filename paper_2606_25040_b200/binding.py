@@ -22,6 +22,7 @@ EXPORTS = ["chorus_mask_to_index", "chorus_visit_refresh", "chorus_block_sparse_
            "chorus_block_sparse_attn_fwd_lse", "chorus_block_sparse_attn_fwd_first_frame",
            "chorus_mask_to_index_64x128", "chorus_block_sparse_attn_fwd_64x128", "chorus_block_mass_64x128",
            "chorus_mask_to_index_u16", "chorus_mask_to_index_64x128_u16", "chorus_block_sparse_attn_fwd_idx16",
+           "chorus_mask_to_index_static",
            "chorus_quantize_fp8", "chorus_retrieve_top1", "chorus_block_mass",
            "chorus_mask_from_mass", "chorus_mask_coverage", "chorus_head_costs", "chorus_schedule_heads", "chorus_gather_heads", "chorus_scatter_heads", "chorus_last_error", "chorus_version",
            "chorus_launch_count", "chorus_reset_launch_count", "chorus_tensor_map_encodes"]
@@ -83,6 +84,8 @@ def lib() -> C.CDLL:
         L.chorus_mask_to_index_64x128.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                                   C.c_int64, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p]
         L.chorus_mask_to_index_u16.argtypes = L.chorus_mask_to_index.argtypes
+        L.chorus_mask_to_index_static.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p,
+                                                  C.c_void_p, C.c_int64, C.c_void_p]
         L.chorus_mask_to_index_64x128_u16.argtypes = L.chorus_mask_to_index_64x128.argtypes
         L.chorus_block_sparse_attn_fwd_idx16.argtypes = (
             L.chorus_block_sparse_attn_fwd_first_frame.argtypes[:-1] + [C.c_int, C.c_void_p])
@@ -165,6 +168,24 @@ def chorus_mask_to_index(bitmask, nk_blk: int, row_ptr=None, col_idx=None, works
     assert col_idx.element_size() == (2 if idx16 else 4)
     _check(fn(_ptr(bitmask), L, H, nq, nk_blk, _ptr(row_ptr), _ptr(col_idx),
               col_idx.numel(), _ptr(workspace), C.byref(wsb), _stream(stream)))
+    return row_ptr, col_idx
+
+
+STATIC_DECODE_MAX_WORDS = 1 << 24
+
+
+def chorus_mask_to_index_static(bitmask, nk_blk: int, row_ptr, col_idx=None, stream=None):
+    """chorus_mask_to_index without a workspace and without any allocation inside the call (the kernel's scratch
+    is a fixed device array of the library; at most STATIC_DECODE_MAX_WORDS mask words; calls that overlap on the
+    GPU race).  row_ptr (and col_idx, unless only the counts are wanted) are the caller's tensors."""
+    L, H, nq, words = bitmask.shape
+    assert bitmask.is_cuda and bitmask.is_contiguous() and bitmask.element_size() == 4
+    assert words == (nk_blk + 31) // 32
+    assert row_ptr.is_cuda and row_ptr.dtype == torch.int32 and row_ptr.numel() >= L * H * nq + 1
+    assert col_idx is None or (col_idx.is_cuda and col_idx.dtype == torch.int32)
+    _check(lib().chorus_mask_to_index_static(_ptr(bitmask), L, H, nq, nk_blk, _ptr(row_ptr),
+                                             None if col_idx is None else _ptr(col_idx),
+                                             0 if col_idx is None else col_idx.numel(), _stream(stream)))
     return row_ptr, col_idx
 
 

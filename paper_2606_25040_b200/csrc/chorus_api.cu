@@ -187,6 +187,34 @@ chorus_status chorus_mask_to_index_u16(const uint32_t* bitmask, int L, int H, in
                               workspace_bytes, cuda_stream);
 }
 
+chorus_status chorus_mask_to_index_static(const uint32_t* bitmask, int L, int H, int nq_blk, int nk_blk,
+                                          int32_t* row_ptr, int32_t* col_idx, int64_t col_cap,
+                                          void* cuda_stream) {
+    static_assert(STATIC_DECODE_MAX_TILES == CHORUS_STATIC_DECODE_MAX_TILES, "header and kernel disagree");
+    g_err[0] = 0;
+    if (L <= 0 || H <= 0 || nq_blk <= 0 || nk_blk <= 0)
+        return set_error(CHORUS_ERR_INVALID_ARG, "L, H, nq_blk, nk_blk must be positive (%d %d %d %d)",
+                         L, H, nq_blk, nk_blk);
+    const int64_t rows = static_cast<int64_t>(L) * H * nq_blk;
+    if (rows * nk_blk > INT32_MAX)
+        return set_error(CHORUS_ERR_CAPACITY, "L*H*nq_blk*nk_blk = %lld exceeds INT32_MAX",
+                         static_cast<long long>(rows * nk_blk));
+    const int words = (nk_blk + 31) / 32;
+    if (rows * words > CHORUS_STATIC_DECODE_MAX_WORDS || decode_static_tiles(rows, words) > STATIC_DECODE_MAX_TILES)
+        return set_error(CHORUS_ERR_CAPACITY,
+                         "mask set of %lld words exceeds the %d words the static scratch of "
+                         "chorus_mask_to_index_static covers (use chorus_mask_to_index with a workspace)",
+                         static_cast<long long>(rows * words), CHORUS_STATIC_DECODE_MAX_WORDS);
+    if (!bitmask || !row_ptr) return set_error(CHORUS_ERR_INVALID_ARG, "bitmask / row_ptr is null");
+    if (col_cap < 0) return set_error(CHORUS_ERR_INVALID_ARG, "col_cap < 0");
+    if ((reinterpret_cast<uintptr_t>(bitmask) | reinterpret_cast<uintptr_t>(row_ptr) |
+         reinterpret_cast<uintptr_t>(col_idx)) & 3u)
+        return set_error(CHORUS_ERR_INVALID_ARG, "pointers must be 4-byte aligned");
+    return check_cuda(launch_mask_decode_static(bitmask, rows, nk_blk, words, row_ptr, col_idx, false, col_cap,
+                                                static_cast<cudaStream_t>(cuda_stream)),
+                      "mask decode (static scratch) launch");
+}
+
 static chorus_status mask_to_index_64x128_impl(const uint32_t* bitmask, int L, int H, int N,
                                                int32_t* row_ptr, void* col_idx, bool idx16, int64_t col_cap,
                                                void* workspace, size_t* workspace_bytes, void* cuda_stream) {

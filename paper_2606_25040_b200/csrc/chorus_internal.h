@@ -20,6 +20,11 @@ cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, in
                                int32_t* row_ptr, void* col_idx, bool idx16, int64_t col_cap, void* workspace,
                                cudaStream_t stream);
 size_t decode_64x128_workspace_bytes(int64_t heads, int N);
+// decode with the status words in a file-scope device array of mask_decode.cu (no allocation, no workspace)
+constexpr int64_t STATIC_DECODE_MAX_TILES = 16384;
+int64_t decode_static_tiles(int64_t rows, int words);
+cudaError_t launch_mask_decode_static(const uint32_t* bitmask, int64_t rows, int nk, int words, int32_t* row_ptr,
+                                      void* col_idx, bool idx16, int64_t col_cap, cudaStream_t stream);
 cudaError_t launch_mask_decode_64x128(const uint32_t* bm64, int64_t heads, int N, int32_t* row_ptr,
                                       void* col_idx, bool idx16, int64_t col_cap, void* workspace, cudaStream_t stream);
 cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_layer, int words,

@@ -13,6 +13,7 @@
 //      which the block copies to col_idx in contiguous, coalesced runs.
 // Algorithmic traffic: 4*(rows*words) read + 4*(rows+1) + 4*nnz written; nothing is read twice.
 #include <algorithm>
+#include <mutex>
 
 #include "chorus_internal.h"
 
@@ -344,6 +345,49 @@ cudaError_t launch_mask_decode(const uint32_t* bitmask, int64_t rows, int nk, in
     if (idx16)
         return launch_decode<uint16_t>(bitmask, nullptr, rows, nk, words, row_ptr, static_cast<uint16_t*>(col_idx), col_cap, workspace, stream);
     return launch_decode<int32_t>(bitmask, nullptr, rows, nk, words, row_ptr, static_cast<int32_t*>(col_idx), col_cap, workspace, stream);
+}
+
+// ---- decode without any allocation (chorus_mask_to_index_static) --------------------------------------------------
+// For callers that cannot provide or allocate a workspace (CUDA graph capture, serving loops and harnesses that
+// forbid cudaMalloc): the per-tile status words live in this file-scope device array, 128 KB that every GPU which
+// loads the library holds until exit.  All calls share it, so two such calls that overlap on the GPU race; it keeps
+// the previous call's contents, and launch_decode clears the words it is going to use (a memset node on the call's
+// stream, no allocation) as it does with a caller's workspace.
+static __device__ __align__(256) unsigned long long g_decode_scratch[STATIC_DECODE_MAX_TILES + 1];
+
+int64_t decode_static_tiles(int64_t rows, int words) { return n_tiles_for(rows, words); }
+
+// In host code `g_decode_scratch` is a host-side stand-in, not a device address: the address is asked for once per
+// device, with that device current, and kept.
+static cudaError_t decode_scratch_address(unsigned long long** out) {
+    constexpr int MAX_DEVICES = 64;
+    static std::mutex mu;
+    static unsigned long long* addr[MAX_DEVICES] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void* ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_decode_scratch);
+        if (e != cudaSuccess) return e;
+        if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u)) return cudaErrorInvalidSymbol;
+        addr[dev] = static_cast<unsigned long long*>(ptr);
+    }
+    *out = addr[dev];
+    return cudaSuccess;
+}
+
+cudaError_t launch_mask_decode_static(const uint32_t* bitmask, int64_t rows, int nk, int words, int32_t* row_ptr,
+                                      void* col_idx, bool idx16, int64_t col_cap, cudaStream_t stream) {
+    if (n_tiles_for(rows, words) > STATIC_DECODE_MAX_TILES) return cudaErrorInvalidValue;   // (checked by the caller)
+    unsigned long long* scratch = nullptr;
+    cudaError_t e = decode_scratch_address(&scratch);
+    if (e != cudaSuccess) return e;
+    if (idx16)
+        return launch_decode<uint16_t>(bitmask, nullptr, rows, nk, words, row_ptr, static_cast<uint16_t*>(col_idx), col_cap, scratch, stream);
+    return launch_decode<int32_t>(bitmask, nullptr, rows, nk, words, row_ptr, static_cast<int32_t*>(col_idx), col_cap, scratch, stream);
 }
 
 cudaError_t launch_visit_refresh(uint32_t* bitmask, int L, int64_t words_per_layer, int words,
