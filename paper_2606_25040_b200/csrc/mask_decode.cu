@@ -8,9 +8,11 @@
 //   2. scans the counts inside the block and gets the number of set bits in front of its tile with
 //      a decoupled look-back over the per-tile status words, 256 at a time (tiles are taken in
 //      ticket order, so a tile only ever waits for tiles that already run);
-//   3. writes row_ptr for every row that begins in the tile; every thread walks the set bits of its
-//      words into a shared-memory staging buffer (before the look-back when the whole tile fits),
-//      which the block copies to col_idx in contiguous, coalesced runs.
+//   3. writes row_ptr for every row that begins in the tile; the set bits of the tile's words are walked into a
+//      shared-memory staging buffer (before the look-back when the whole tile fits) - in the plain geometry after
+//      a counting sort of the words by popcount, so that the lanes of a warp walk equally long words - which the
+//      block copies to col_idx in contiguous, coalesced runs.  Entries that fit 16 bits are staged in 16-bit
+//      slots (24 KB instead of 44 KB of shared memory: eight resident blocks per SM instead of five).
 // Algorithmic traffic: 4*(rows*words) read + 4*(rows+1) + 4*nnz written; nothing is read twice.
 #include <algorithm>
 #include <mutex>
@@ -22,7 +24,13 @@ namespace {
 
 constexpr int DEC_THREADS = 256;
 constexpr int DEC_WARPS = DEC_THREADS / 32;
-constexpr int STAGE = 9216;                                      // col_idx entries staged per round
+#ifndef DEC_BLOCKS16
+#define DEC_BLOCKS16 8                                           // resident blocks per SM aimed at with 16-bit slots (32 registers)
+#endif
+// col_idx entries staged per round: 44 KB of 32-bit or 24 KB of 16-bit slots (entries that fit 16 bits are staged
+// in 16 bits: more resident blocks per SM)
+template <typename StageT>
+constexpr int stage_entries() { return sizeof(StageT) == 2 ? 12288 : 11264; }
 
 // Staging-buffer slot of entry e: the low five bits are XORed with the next five, so that threads whose runs
 // start 8, 16 or 32 entries apart (25 %, 50 %, full density) hit different banks when they all write their
@@ -32,14 +40,14 @@ __device__ __forceinline__ int slot(int e) { return e ^ ((e >> 5) & 31); }
 // The set bits of x, ascending, into the staging buffer from entry e on.  Walked from the top bit down into
 // descending slots: the position of the highest set bit is ONE instruction (FLO), where the lowest one costs a
 // bit reversal as well.  val(b) gives the entry of bit b.
-template <typename F>
-__device__ __forceinline__ void walk_word(uint32_t x, int e, int32_t* s_stage, F val) {
+template <typename StageT, typename F>
+__device__ __forceinline__ void walk_word(uint32_t x, int e, StageT* s_stage, F val) {
     int pos = e + __popc(x) - 1;
     while (x) {
         int b;
         asm("bfind.u32 %0, %1;" : "=r"(b) : "r"(x));   // one FLO; `31 - __clz(x)` compiles to a clz and its way back
         x ^= 1u << b;
-        s_stage[slot(pos)] = val(b);
+        s_stage[slot(pos)] = static_cast<StageT>(val(b));
         --pos;
     }
 }
@@ -103,22 +111,43 @@ __device__ __forceinline__ IdxT out_entry(int32_t e) {
     if constexpr (kGeo) return static_cast<IdxT>((u & 0x3fffu) | ((u >> 30) << 14));
     return static_cast<IdxT>(u);
 }
+// the same on the way INTO the staging buffer (StageT 16-bit: the conversion happens here) and out of it
+template <typename StageT, bool kGeo>
+__device__ __forceinline__ StageT stage_entry(int32_t e) { return out_entry<StageT, kGeo>(e); }
+template <typename IdxT, typename StageT, bool kGeo>
+__device__ __forceinline__ IdxT unstage_entry(StageT v) {
+    if constexpr (sizeof(StageT) == 2) return static_cast<IdxT>(v);     // already in its final form (zero-extended)
+    else return out_entry<IdxT, kGeo>(static_cast<int32_t>(v));
+}
 
 // WPT consecutive words per thread: 4 for large mask sets (fewer scans, divisions and status words per
 // word), 1 for a single layer (more, smaller tiles: one 480p layer is only 160 K words)
-template <int WPT, bool kGeo, typename IdxT>
-__global__ void __launch_bounds__(DEC_THREADS)
+template <int WPT, bool kGeo, typename IdxT, typename StageT>
+__global__ void __launch_bounds__(DEC_THREADS, sizeof(StageT) == 2 ? DEC_BLOCKS16 : 5)
 decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, int words,
                     int32_t* __restrict__ row_ptr, IdxT* __restrict__ col_idx, int64_t col_cap,
                     unsigned long long* __restrict__ status /* [0] = ticket counter, [1 + t] = tile t */,
                     const GeoSrc geo) {
-    __shared__ int32_t s_stage[STAGE];           // entry e at slot(e)
+    static_assert(sizeof(StageT) == 4 || sizeof(IdxT) == 2 || !kGeo, "flagged 32-bit entries need 32-bit slots");
+    constexpr int STAGE = stage_entries<StageT>();
+    __shared__ __align__(16) unsigned char s_raw[STAGE * sizeof(StageT)];
+    StageT* s_stage = reinterpret_cast<StageT*>(s_raw);          // entry e at slot(e)
     __shared__ int s_warp[DEC_WARPS];
     __shared__ int2 s_look[DEC_WARPS];
     __shared__ int s_tile, s_base;
     constexpr int TILE_WORDS = DEC_THREADS * WPT;
+    // words of the tile in descending order of their popcount (see "balanced walk" below): the word and
+    // (staging offset | word-in-row << 14); s_bkt: per popcount 32..1 a counter, then the bucket's first position
+    // They live in the tail of the staging buffer, which such a tile does not reach.
+    constexpr bool kSort = !kGeo;
+    constexpr int SORT_MAX = STAGE - 2 * TILE_WORDS * 4 / static_cast<int>(sizeof(StageT));   // most entries of a tile walked sorted
+    static_assert(SORT_MAX % 32 == 0 && SORT_MAX >= 8192, "sorted walk must cover a 1024-word tile at 25 % density");
+    uint32_t* s_wx = reinterpret_cast<uint32_t*>(s_stage + SORT_MAX);
+    uint32_t* s_wm = s_wx + TILE_WORDS;
+    __shared__ int s_bkt[33];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) s_tile = static_cast<int>(atomicAdd(status, 1ull));
+    if (threadIdx.x < 33) s_bkt[threadIdx.x] = 0;
     __syncthreads();
     const int tile = s_tile;
     // all word indices fit 32 bits: rows * nk <= INT32_MAX is checked by the caller
@@ -152,6 +181,13 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
             if (++wr == words) { wr = 0; ++r; }
         }
     }
+    // (histogram of the words' popcounts for the balanced walk below; complete at the next barrier)
+    int rank[WPT];
+#pragma unroll
+    for (int i = 0; i < WPT; ++i) {
+        const int pc = __popc(v[i]);
+        rank[i] = (kSort && pc) ? atomicAdd(&s_bkt[32 - pc], 1) : 0;
+    }
     // 2a/2b. one exclusive scan of the thread counts inside the block
     int inc = cnt;
 #pragma unroll
@@ -177,16 +213,59 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
         if (threadIdx.x == 0)
             st_status(mine, (tile == 0 ? ST_INC : ST_AGG) | static_cast<uint32_t>(tile_total));
         // While the predecessors publish, expand: the staging offsets do not need the global base.
-        if (fast) {
+        // Balanced walk.  A warp walks as long as its fullest lane, and popcounts differ a lot (the all-kept frame-0
+        // blocks of every row's first word, L81; binomial spread elsewhere): with every thread walking its own
+        // words the tile costs 2.3 x the warp iterations of a balanced walk.  The tile's non-empty words are
+        // therefore counting-sorted by popcount in shared memory (33 buckets, descending) and thread t walks the
+        // sorted words t, t + 256, ...: the 32 lanes of a warp get words of (nearly) the same popcount.  A word
+        // carries its staging offset and its position in the row along, so where it is walked does not matter.
+        if (fast && kSort && tile_total <= SORT_MAX) {
+            static_assert(STAGE <= (1 << 14), "staging offset must fit 14 bits");
+            // every warp scans the 32 buckets (popcount 32, 31, .., 1) for itself: no second barrier
+            const int c = s_bkt[lane];
+            int incl = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int u = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += u;
+            }
+            const int start = incl - c;
+            const int n_nz = __shfl_sync(0xffffffffu, incl, 31);   // non-empty words of the tile
+            {
+                int e = off, wr = win0;
+#pragma unroll
+                for (int i = 0; i < WPT; ++i) {
+                    const int pc = __popc(v[i]);
+                    const int st = __shfl_sync(0xffffffffu, start, (32 - pc) & 31);
+                    if (pc) {
+                        const int pos = st + rank[i];
+                        s_wx[pos] = v[i];
+                        s_wm[pos] = static_cast<uint32_t>(e) | (static_cast<uint32_t>(wr) << 14);
+                    }
+                    e += pc;
+                    if (++wr == words) wr = 0;
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int i = 0; i < WPT; ++i) {
+                const int pos = i * DEC_THREADS + static_cast<int>(threadIdx.x);
+                if (pos < n_nz) {
+                    const uint32_t x = s_wx[pos], meta = s_wm[pos];
+                    const int kb0 = static_cast<int>(meta >> 14) * 32;
+                    walk_word(x, static_cast<int>(meta & 0x3fffu), s_stage, [&](int b) { return stage_entry<StageT, kGeo>(kb0 + b); });
+                }
+            }
+        } else if (fast) {
             int e = off, wr = win0;
 #pragma unroll
             for (int i = 0; i < WPT; ++i) {
                 const int kb0 = wr * 32;
                 if constexpr (kGeo) {
                     const uint32_t gu = fu[i], gl = fl[i];
-                    walk_word(v[i], e, s_stage, [&](int b) { return geo_entry(kb0 + b, b, gu, gl); });
+                    walk_word(v[i], e, s_stage, [&](int b) { return stage_entry<StageT, kGeo>(geo_entry(kb0 + b, b, gu, gl)); });
                 } else {
-                    walk_word(v[i], e, s_stage, [&](int b) { return kb0 + b; });
+                    walk_word(v[i], e, s_stage, [&](int b) { return stage_entry<StageT, kGeo>(kb0 + b); });
                 }
                 e += __popc(v[i]);
                 if (++wr == words) wr = 0;
@@ -239,7 +318,7 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
         const int n_out = static_cast<int>(min(static_cast<int64_t>(tile_total), max(col_cap - base, static_cast<int64_t>(0))));
         IdxT* dst = col_idx + base;
 #pragma unroll 4
-        for (int t = threadIdx.x; t < n_out; t += DEC_THREADS) dst[t] = out_entry<IdxT, kGeo>(s_stage[slot(t)]);
+        for (int t = threadIdx.x; t < n_out; t += DEC_THREADS) dst[t] = unstage_entry<IdxT, StageT, kGeo>(s_stage[slot(t)]);
         return;
     }
     // 3b. a fuller tile (WPT > 1 only): WPT rounds of one word per thread, so that every thread walks
@@ -248,8 +327,8 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
     // sits behind the largest round in the staging buffer.
     if constexpr (WPT > 1) {
         constexpr int ROUND_MAX = DEC_THREADS * 32;
-        static_assert(ROUND_MAX + TILE_WORDS <= STAGE, "staging buffer too small for a round plus the offset table");
-        int* s_woff = s_stage + ROUND_MAX;
+        static_assert(ROUND_MAX * sizeof(StageT) + TILE_WORDS * 4 <= sizeof(s_raw), "staging buffer too small for a round plus the offset table");
+        int* s_woff = reinterpret_cast<int*>(s_raw + ROUND_MAX * sizeof(StageT));
         {
             int o = off;
 #pragma unroll
@@ -272,13 +351,13 @@ decode_tiles_kernel(const uint32_t* __restrict__ bitmask, int64_t rows, int nk, 
             if (wr == words - 1) x &= last_mask;
             const int e = s_woff[j] - lo;
             const int kb0 = wr * 32;
-            if constexpr (kGeo) walk_word(x, e, s_stage, [&](int b) { return geo_entry(kb0 + b, b, gu, gl); });
-            else walk_word(x, e, s_stage, [&](int b) { return kb0 + b; });
+            if constexpr (kGeo) walk_word(x, e, s_stage, [&](int b) { return stage_entry<StageT, kGeo>(geo_entry(kb0 + b, b, gu, gl)); });
+            else walk_word(x, e, s_stage, [&](int b) { return stage_entry<StageT, kGeo>(kb0 + b); });
             __syncthreads();
             const int n_out = static_cast<int>(min(static_cast<int64_t>(hi - lo), max(col_cap - base - lo, static_cast<int64_t>(0))));
             IdxT* dst = col_idx + base + lo;
 #pragma unroll 4
-            for (int t = threadIdx.x; t < n_out; t += DEC_THREADS) dst[t] = out_entry<IdxT, kGeo>(s_stage[slot(t)]);
+            for (int t = threadIdx.x; t < n_out; t += DEC_THREADS) dst[t] = unstage_entry<IdxT, StageT, kGeo>(s_stage[slot(t)]);
             __syncthreads();
         }
     }
@@ -317,6 +396,10 @@ size_t decode_workspace_bytes(int64_t rows, int words) {
     return static_cast<size_t>(n_tiles_for(rows, words) + 1) * sizeof(unsigned long long) + 8;
 }
 
+template <int V> struct IntTag { static constexpr int value = V; };
+template <bool V> struct BoolTag { static constexpr bool value = V; };
+template <typename T> struct TypeTag { using type = T; };
+
 template <typename IdxT>
 static cudaError_t launch_decode(const uint32_t* bitmask, const GeoSrc* geo, int64_t rows, int nk, int words,
                                  int32_t* row_ptr, IdxT* col_idx, int64_t col_cap, void* workspace,
@@ -328,12 +411,32 @@ static cudaError_t launch_decode(const uint32_t* bitmask, const GeoSrc* geo, int
     const unsigned grid = static_cast<unsigned>(nt);
     const bool one = wpt_for(rows * words) == 1;
     const GeoSrc g = geo ? *geo : GeoSrc{nullptr, 0, 0, 0, 0};
+    // entries that fit 16 bits are staged in 16-bit slots: always for 16-bit output; for 32-bit output when they carry
+    // no flags (plain geometry) and nk <= 65536
+    auto go = [&](auto wpt_tag, auto geo_tag, auto stage_tag) {
+        constexpr int W = decltype(wpt_tag)::value;
+        constexpr bool G = decltype(geo_tag)::value;
+        using StageT = typename decltype(stage_tag)::type;
+        decode_tiles_kernel<W, G, IdxT, StageT><<<grid, DEC_THREADS, 0, stream>>>(geo ? nullptr : bitmask, rows, nk, words, row_ptr,
+                                                                                col_idx, col_cap, status, g);
+    };
+    const bool stage16 = sizeof(IdxT) == 2 || (!geo && nk <= 65536);
     if (geo) {
-        if (one) decode_tiles_kernel<1, true, IdxT><<<grid, DEC_THREADS, 0, stream>>>(nullptr, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
-        else decode_tiles_kernel<4, true, IdxT><<<grid, DEC_THREADS, 0, stream>>>(nullptr, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+        if constexpr (sizeof(IdxT) == 2) {
+            if (one) go(IntTag<1>{}, BoolTag<true>{}, TypeTag<uint16_t>{});
+            else go(IntTag<4>{}, BoolTag<true>{}, TypeTag<uint16_t>{});
+        } else {
+            if (one) go(IntTag<1>{}, BoolTag<true>{}, TypeTag<int32_t>{});
+            else go(IntTag<4>{}, BoolTag<true>{}, TypeTag<int32_t>{});
+        }
+    } else if (stage16) {
+        if (one) go(IntTag<1>{}, BoolTag<false>{}, TypeTag<uint16_t>{});
+        else go(IntTag<4>{}, BoolTag<false>{}, TypeTag<uint16_t>{});
     } else {
-        if (one) decode_tiles_kernel<1, false, IdxT><<<grid, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
-        else decode_tiles_kernel<4, false, IdxT><<<grid, DEC_THREADS, 0, stream>>>(bitmask, rows, nk, words, row_ptr, col_idx, col_cap, status, g);
+        if constexpr (sizeof(IdxT) == 4) {
+            if (one) go(IntTag<1>{}, BoolTag<false>{}, TypeTag<int32_t>{});
+            else go(IntTag<4>{}, BoolTag<false>{}, TypeTag<int32_t>{});
+        }
     }
     count_launch(1);
     return cudaGetLastError();
