@@ -96,6 +96,21 @@ def test_large_mask_set_four_words_per_thread():
     assert np.array_equal(got[:cap], ci_o[:cap]) and np.all(got[cap:] == -7)
 
 
+@pytest.mark.parametrize("nq", [40, 500])
+def test_more_than_65536_key_blocks_take_32_bit_staging_slots(nq):
+    """nk > 65536: the entries do not fit the 16-bit staging slots of the usual path, so the kernel instantiation
+    with 32-bit slots runs, one word per thread (nq = 40) and four (nq = 500: >= 2^20 words); row
+    densities from 0 to 0.6 cover its sorted walk, its per-thread walk and its rounds."""
+    nk = 70001
+    g = np.random.default_rng(nq)
+    rho = g.choice([0.0, 0.02, 0.2, 0.3, 0.6], size=nq)
+    bm = W.pack_bits((g.random((nq, nk)) < rho[:, None]).reshape(1, 1, nq, nk))
+    bm[..., -1] |= np.uint32((0xFFFFFFFF << (nk % 32)) & 0xFFFFFFFF)
+    assert (bm.size >= 1 << 20) == (nq == 500)
+    rp, ci = check(bm, nk)
+    assert int(ci.max().item()) > 65536
+
+
 def test_visit_refresh_matches_oracle():
     nk, nq, H, L = 45, 3, 2, 19
     g = np.random.default_rng(3)
