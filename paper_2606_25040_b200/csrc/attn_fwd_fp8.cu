@@ -56,24 +56,16 @@ constexpr uint32_t PV_N = 144;          // 128 channels + 16 ones columns (M = 1
 // P = exp2(x - m_ref + 5): e4m3 (max 448, smallest normal 2^-6) keeps probabilities down to 2^-11 of the row
 // maximum as normal numbers while P <= 2^8 holds under the lazy-rescale threshold of 2^3.
 constexpr float P_SHIFT = 5.0f, RESCALE_THRESHOLD = 3.0f;
-// The exponentials of a pair are split between two units, by element pair (index mod 8; the masks can be set at
-// build time for measurements):
+// The exponentials of a pair are split between two units, by element pair (index mod 8):
 //   LIN_MASK   every other pair: the piecewise-linear 2^x read off the score's own bits on the ALU / FMA pipes.
 //              t = x + 1.5 * 2^15 leaves round(x * 2^8) in the low mantissa bits of t, and (bits(t) << 15) + LIN_K is
-//              the float 2^floor(x) * (1 + frac(x) - d): one FMNMX (clamp at 2^-126) and one integer multiply-add per
+//              the float 2^floor(x) * (1 + frac(x) - d): one FMNMX (clamp at 2^-126) and one integer shift-add per
 //              element after the FFMA2 that every path needs.  d = 0.0564 centres the error: -2.8 % .. +2.0 % with
 //              mean 0 over frac(x), next to the +-3.1 % of the e4m3 rounding that follows; the row sums are taken by
 //              the tensor cores from the same P, so numerator and denominator stay consistent and unbiased.
-//   POLY_MASK  (none by default) the degree-2 polynomial exp2 on the FMA pipe, relative error 1.7e-3
 //   the rest   MUFU.EX2, one warp instruction per 8 cycles and scheduler: the unit that bounded the kernel
-#ifndef FP8_POLY_MASK
-#define FP8_POLY_MASK 0x00u
-#endif
-#ifndef FP8_LIN_MASK
-#define FP8_LIN_MASK 0x55u
-#endif
-constexpr uint32_t POLY_MASK = FP8_POLY_MASK;
-constexpr uint32_t LIN_MASK = FP8_LIN_MASK;
+// (4 of 8 is the measured optimum: DESIGN.md section 6.5)
+constexpr uint32_t LIN_MASK = 0x55u;
 constexpr float LIN_C = 49152.0f;                                  // 1.5 * 2^15: ulp 2^-8
 constexpr float LIN_LO = LIN_C - 126.0f;                           // 2^-126: rounds to the e4m3 code 0
 constexpr int LIN_K = static_cast<int>((127u << 23) - 473118u - (0x47400000u << 15));
@@ -398,7 +390,6 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                             return make_float2(__int_as_float((ix << 15) + LIN_K), __int_as_float((iy << 15) + LIN_K));
                         }
                         const float2 x = ffma2(sv, q < 32 ? sl2a_2 : sl2b_2, negm_2);
-                        if ((POLY_MASK >> (q & 7)) & 1u) return exp2_poly2<2>(x);
                         return make_float2(ex2(x.x), ex2(x.y));
                     };
 #pragma unroll

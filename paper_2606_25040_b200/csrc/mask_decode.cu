@@ -24,9 +24,7 @@ namespace {
 
 constexpr int DEC_THREADS = 256;
 constexpr int DEC_WARPS = DEC_THREADS / 32;
-#ifndef DEC_BLOCKS16
-#define DEC_BLOCKS16 8                                           // resident blocks per SM aimed at with 16-bit slots (32 registers)
-#endif
+constexpr int DEC_BLOCKS16 = 8;                                  // resident blocks per SM aimed at with 16-bit slots (32 registers)
 // col_idx entries staged per round: 44 KB of 32-bit or 24 KB of 16-bit slots (entries that fit 16 bits are staged
 // in 16 bits: more resident blocks per SM)
 template <typename StageT>
