@@ -60,7 +60,7 @@ constexpr float P_SHIFT = 5.0f, RESCALE_THRESHOLD = 3.0f;
 //   LIN_MASK   every other pair: the piecewise-linear 2^x read off the score's own bits on the ALU / FMA pipes.
 //              t = x + 1.5 * 2^15 leaves round(x * 2^8) in the low mantissa bits of t, and (bits(t) << 15) + LIN_K is
 //              the float 2^floor(x) * (1 + frac(x) - d): one FMNMX (clamp at 2^-126) and one integer shift-add per
-//              element after the FFMA2 that every path needs.  d = 0.0564 centres the error: -2.8 % .. +2.0 % with
+//              element after the FFMA2 that every path needs.  d = 0.0564 makes the error -3.8 % .. +2.1 % with
 //              mean 0 over frac(x), next to the +-3.1 % of the e4m3 rounding that follows; the row sums are taken by
 //              the tensor cores from the same P, so numerator and denominator stay consistent and unbiased.
 //   the rest   MUFU.EX2, one warp instruction per 8 cycles and scheduler: the unit that bounded the kernel
