@@ -17,7 +17,8 @@
 //     e4m3-rounded weights that multiply V (so a row dominated by one key does not inherit the 2^-4 rounding of its
 //     weight), rescaled together with O on the lazy-rescale path.  This removes the e4m3 -> f16 unpack, the HADD2
 //     accumulation and the (m, l) exchange between the two softmax parities of the epilogue.
-//   warp 8        TMA producer: Q tile once per item, K / V pairs into two rings of four 16 KB stages
+//   warp 8        TMA producer: Q tile once per item, K / V pairs into two rings of four 16 KB stages; the pair's
+//                 col_idx entries and K scales into a small ring for the softmax warps
 //   warp 9        MMA issuer: S = Q K^T (kind::f8f6f4, M 128, N 128, K 128) into S[g % 2]; O += P V (P the TMEM A
 //                 operand, V an MN-major B operand, N = 144 with the ones columns) two pairs behind
 //   warps 0-3     softmax of the even pairs of an item; warps 4-7 of the odd pairs (one query row per thread)
@@ -34,13 +35,20 @@ using namespace ptx;
 using namespace attn;
 
 constexpr int KSTAGES = 4, VSTAGES = 4, SBUFS = 2, PBUFS = 3;
+// What the softmax warps need to know about a pair - its two col_idx entries and the K scales of its two key blocks -
+// is fetched ONCE, by the producer warp (which has the entries anyway), and handed over in shared memory: entry
+// g % PAIR_RING, written before the pair's K tiles are requested.  The producer is at most KSTAGES pairs ahead of the
+// Q K^T issue and that at most SBUFS pairs ahead of the last softmax warp's read of S, which follows its read of the
+// entry: 8 > 4 + 2 entries are never overwritten early.
+constexpr uint32_t PAIR_RING = 8;
 constexpr uint32_t TILE = 16384;        // one pair stage: [128 keys][128 B] = two 64-key tiles of 128 e4m3 channels
 constexpr uint32_t HALF = 8192;         // the second tile of a pair
 // shared memory map (bytes from a 1024-aligned base).  The ones slab lies ABOVE every V stage: the B descriptor of
 // a P V step reaches it as the second 128-byte column block of its operand (leading-dimension byte offset).
 constexpr uint32_t SQ_OFF = 0, SK_OFF = TILE, SV_OFF = SK_OFF + KSTAGES * TILE, ONES_OFF = SV_OFF + VSTAGES * TILE,
                    ONES_BYTES = 4096,   // [32 keys][128 B] of e4m3 1.0: one K = 32 MMA step's worth
-                   SO_OFF = ONES_OFF + ONES_BYTES, XCH_OFF = SO_OFF + 32768, BAR_OFF = XCH_OFF + 512,
+                   SO_OFF = ONES_OFF + ONES_BYTES, XCH_OFF = SO_OFF + 32768, PR_OFF = XCH_OFF + 512,
+                   BAR_OFF = PR_OFF + PAIR_RING * 16,
                    SMEM_BYTES = BAR_OFF + 384;
 static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB per-CTA shared memory of sm_100");
 // mbarrier slots
@@ -90,6 +98,7 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
     auto bar = [&](uint32_t i) { return bars + 8u * i; };
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gbase + BAR_OFF + 8 * B_COUNT);
     volatile float* xm = reinterpret_cast<volatile float*>(gbase + XCH_OFF);   // [128] m_ref hand-off
+    const uint32_t pair_ring = base + PR_OFF;                                   // [PAIR_RING] {entry a, entry b, k scale a, b}
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_items = p.B * p.H * p.nq;
@@ -138,20 +147,28 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                     tma_load_4d(sQ, &tmQ, bar(B_Q_FULL), 0, it.qb * BQ, it.h, it.b);
                 }
                 __syncwarp();
-                // the key-block indices of 16 pairs are fetched with one coalesced load
+                const float* ksc = p.k_scale + (static_cast<int64_t>(it.b) * p.H + it.h) * ((p.N + 127) >> 7);
+                // the key-block indices of 16 pairs are fetched with one coalesced load, their K scales with a second
                 for (int j0 = 0; j0 < it.np; j0 += 16) {
                     const int t = 2 * j0 + lane;
-                    int mine = (t < it.nt) ? ld_col(p, it.r0 + t) : 0;
-                    if constexpr (kHalf) mine &= 0x3fffffff;
+                    const int raw = (t < it.nt) ? ld_col(p, it.r0 + t) : 0;     // kHalf: with the per-half flags
+                    const int mine = kHalf ? (raw & 0x3fffffff) : raw;
+                    const float mysc = (t < it.nt) ? __ldg(ksc + (mine >> 1)) : 0.f;
                     const int jn = min(16, it.np - j0);
                     for (int jl = 0; jl < jn; ++jl, ++g) {
                         const int ntile = (2 * (j0 + jl) + 1 < it.nt) ? 2 : 1;
                         const int kb0 = __shfl_sync(0xffffffffu, mine, 2 * jl);
                         const int kb1 = __shfl_sync(0xffffffffu, mine, 2 * jl + 1);
+                        const int raw0 = kHalf ? __shfl_sync(0xffffffffu, raw, 2 * jl) : kb0;
+                        const int raw1 = kHalf ? __shfl_sync(0xffffffffu, raw, 2 * jl + 1) : kb1;
+                        const float sc0 = __shfl_sync(0xffffffffu, mysc, 2 * jl);
+                        const float sc1 = __shfl_sync(0xffffffffu, mysc, 2 * jl + 1);
                         {
                             const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1;
                             mbar_wait(bar(B_K_EMPTY + st), ph ^ 1);
                             if (elect_one()) {
+                                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(pair_ring + (g % PAIR_RING) * 16),
+                                             "r"(raw0), "r"(raw1), "r"(__float_as_int(sc0)), "r"(__float_as_int(sc1)) : "memory");
                                 mbar_arrive_expect_tx(bar(B_K_FULL + st), ntile * HALF);
                                 const uint32_t dst = sK + st * TILE;
                                 tma_load_4d(dst, &tmK, bar(B_K_FULL + st), 0, kb0 * BK, it.h, it.b);
@@ -257,20 +274,20 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
             const Item it = get_item(p, idx);
             float m_ref = -INFINITY;
             // scores are (q8 . k8) * s_q[qb] * s_k[kb / 2] (R10); the per-tile factor is folded into the
-            // exp2 FMA constant.  The key-block indices of this parity's NEXT pair are fetched one pair ahead.
+            // exp2 FMA constant.  The pair's entries and K scales come from the producer warp (pair ring).
             const int64_t sbase = (static_cast<int64_t>(it.b) * p.H + it.h) * nsb;
             const float qsl2 = p.scale_log2 * __ldg(p.q_scale + sbase + it.qb);
-            const float* ksc = p.k_scale + sbase;
-            int kba_next = 0, kbb_next = 0;
-            if (2 * sm < it.nt) kba_next = ld_col(p, it.r0 + 2 * sm);
-            if (2 * sm + 1 < it.nt) kbb_next = ld_col(p, it.r0 + 2 * sm + 1);
             for (int j = sm; j < it.np; j += 2) {
                 const uint32_t g = g0 + j, sb = g % SBUFS, pb = g % PBUFS;
                 const uint32_t tS = tlane + TM_S + sb * 128, tP = tlane + TM_P + pb * 32;
                 int va = BK, vb = BK;            // valid keys in the two tiles of the pair
-                int kba = kba_next, kbb = kbb_next;
-                if (2 * (j + 2) < it.nt) kba_next = ld_col(p, it.r0 + 2 * (j + 2));
-                if (2 * (j + 2) + 1 < it.nt) kbb_next = ld_col(p, it.r0 + 2 * (j + 2) + 1);
+                // S of the pair is complete; its ring entry was written before its K tiles were even requested
+                mbar_wait(bar(B_S_FULL + sb), (g / SBUFS) & 1);
+                tc_fence_after();
+                int kba, kbb;
+                float ska, skb;
+                asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(kba), "=r"(kbb), "=f"(ska), "=f"(skb)
+                             : "r"(pair_ring + (g % PAIR_RING) * 16) : "memory");
                 uint32_t skip_a = 0u, skip_b = 0u;   // kHalf: this warp's rows do not keep tile a / b
                 if constexpr (kHalf) {
                     const int hb = 30 + (wq >> 1);
@@ -279,8 +296,8 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                     kba &= 0x3fffffff;
                     kbb &= 0x3fffffff;
                 }
-                float sl2a = qsl2 * __ldg(ksc + (kba >> 1));
-                float sl2b = qsl2 * __ldg(ksc + (kbb >> 1));
+                float sl2a = qsl2 * ska;
+                float sl2b = qsl2 * skb;
                 // kBeta: a tile inside the first frame takes beta in its scale factor; the one tile that straddles
                 // n_first takes it per column (fa / fb leading columns) in the masked body
                 int fa = 0, fb = 0;
@@ -300,8 +317,6 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                 }
                 // ---- the 128 scores of the row into registers; the S buffer is free again at once ----
                 uint32_t s[128];
-                mbar_wait(bar(B_S_FULL + sb), (g / SBUFS) & 1);
-                tc_fence_after();
                 tmem_ld32(tS, reinterpret_cast<uint32_t(&)[32]>(s[0]));
                 tmem_ld32(tS + 32, reinterpret_cast<uint32_t(&)[32]>(s[32]));
                 tmem_ld32(tS + 64, reinterpret_cast<uint32_t(&)[32]>(s[64]));
