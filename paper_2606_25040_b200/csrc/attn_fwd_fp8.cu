@@ -240,12 +240,15 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                             const uint32_t tP = tmem + TM_P + pb * 32, tO = tmem + TM_O;
                             const uint32_t vst = sV + st * TILE;
                             const int steps = two ? 4 : 2;           // 32 keys x 128 B per step
-                            for (int ks = 0; ks < steps; ++ks) {
-                                const uint32_t vaddr = vst + ks * 4096;
-                                // columns 128..143 of B come from the ones slab: leading-dimension offset = its distance
-                                const uint64_t dV = smem_desc_sw128(vaddr, sOnes - vaddr, 1024);
-                                mma_f8_ts(tO, tP + ks * 8, dV, IDESC_PV, (jp > 0) || (ks > 0));
-                            }
+                            // columns 128..143 of B come from the ones slab: leading-dimension offset = its distance.
+                            // A step further down the tile adds 4096 B to the start address and takes them off the
+                            // offset: one 64-bit constant on the descriptor (both fields stay inside their bits).
+                            const uint64_t dV0 = smem_desc_sw128(vst, sOnes - vst, 1024);
+                            constexpr uint64_t DV_STEP = static_cast<uint64_t>(256) - (static_cast<uint64_t>(256) << 16);
+#pragma unroll
+                            for (int ks = 0; ks < 4; ++ks)
+                                if (ks < steps)
+                                    mma_f8_ts(tO, tP + ks * 8, dV0 + static_cast<uint64_t>(ks) * DV_STEP, IDESC_PV, (jp > 0) || (ks > 0));
                             tc_commit(bar(B_V_EMPTY + st));
                             tc_commit(bar(B_PV_DONE + pb));
                             if (jp == it.np - 1) tc_commit(bar(B_ITEM_DONE));
