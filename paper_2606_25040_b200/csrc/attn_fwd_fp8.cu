@@ -19,8 +19,10 @@
 //     accumulation and the (m, l) exchange between the two softmax parities of the epilogue.
 //   warp 8        TMA producer: Q tile once per item, K / V pairs into two rings of four 16 KB stages; the pair's
 //                 col_idx entries and K scales into a small ring for the softmax warps
-//   warp 9        MMA issuer: S = Q K^T (kind::f8f6f4, M 128, N 128, K 128) into S[g % 2]; O += P V (P the TMEM A
-//                 operand, V an MN-major B operand, N = 144 with the ones columns) two pairs behind
+//   warp 9        issues S = Q K^T (kind::f8f6f4, M 128, N 128, K 128) into S[g % 2], as soon as the buffer is free
+//   warp 10       issues O += P V (P the TMEM A operand, V an MN-major B operand, N = 144 with the ones columns).
+//                 Two issuing warps on two schedulers: either one's ~80 instructions per pair share a scheduler
+//                 with two softmax warps, and the slowest of the four lane quarters sets the pace of a pair
 //   warps 0-3     softmax of the even pairs of an item; warps 4-7 of the odd pairs (one query row per thread)
 // TMEM (512 columns): O 0..143 (128 channels + 16 copies of the row sum), S0 160.., S1 288.., P0 416, P1 448,
 // P2 480.  O is rescaled lazily: only when a row maximum exceeds the reference by more than 2^3.
@@ -113,7 +115,7 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
         for (int i = 0; i < PBUFS; ++i) { mbar_init(bar(B_P_READY + i), 4); mbar_init(bar(B_PV_DONE + i), 1); }
         mbar_init(bar(B_ITEM_DONE), 1);
         mbar_init(bar(B_O_FREE), 8);
-        for (int i = 0; i < ITEM_RING; ++i) { mbar_init(bar(B_IT_FULL + i), 1); mbar_init(bar(B_IT_EMPTY + i), 9); }   // MMA warp + 8 softmax warps
+        for (int i = 0; i < ITEM_RING; ++i) { mbar_init(bar(B_IT_FULL + i), 1); mbar_init(bar(B_IT_EMPTY + i), 10); }   // two MMA warps + 8 softmax warps
         fence_mbar_init();
     }
     // the ones slab: e4m3 1.0 = 0x38 in every byte (constant, so the 128-byte swizzle does not matter)
@@ -195,8 +197,6 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
             // kind::f8f6f4, format 0 = e4m3.  P V: B (= V and the ones slab) is MN-major, N = 144.
             constexpr uint32_t IDESC_S128 = make_idesc(0, 0, 128, 128, 0, 0);
             constexpr uint32_t IDESC_S64 = make_idesc(0, 0, 128, 64, 0, 0);
-            constexpr uint32_t IDESC_PV = make_idesc(0, 0, 128, PV_N, 0, 1);
-            constexpr int AHEAD = 2;        // QK^T runs this many pairs ahead of P V in the issue order
             const uint64_t dQ = smem_desc_sw128(sQ, 16, 1024);
             const uint64_t dK = smem_desc_sw128(sK, 16, 1024);
             uint32_t g0 = 0, icnt = 0;      // pairs before this item, non-empty items so far
@@ -206,8 +206,8 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                 const Item it = get_item_uniform(p, idx);
                 if (it.nt == 0) continue;
                 mbar_wait(bar(B_Q_FULL), icnt & 1);
-                for (int jj = 0; jj < it.np + AHEAD; ++jj) {
-                    if (jj < it.np) {   // S[g % 2] = Q K^T of pair jj
+                for (int jj = 0; jj < it.np; ++jj) {
+                    {   // S[g % 2] = Q K^T of pair jj
                         const uint32_t g = g0 + jj;
                         const uint32_t st = g % KSTAGES, ph = (g / KSTAGES) & 1, sb = g % SBUFS;
                         const bool two = 2 * jj + 1 < it.nt;
@@ -227,8 +227,20 @@ attn_fwd_fp8_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                         }
                         __syncwarp();
                     }
-                    if (jj >= AHEAD) {      // O += P V of pair jj - AHEAD
-                        const int jp = jj - AHEAD;
+                }
+                g0 += it.np;
+                ++icnt;
+            }
+        } else if (warp == MMA_WARP + 1) {
+            constexpr uint32_t IDESC_PV = make_idesc(0, 0, 128, PV_N, 0, 1);
+            uint32_t g0 = 0, icnt = 0;
+            for (uint32_t kit = 0;; ++kit) {
+                const int idx = item_take(ring, kit);
+                if (idx < 0) break;
+                const Item it = get_item_uniform(p, idx);
+                if (it.nt == 0) continue;
+                for (int jp = 0; jp < it.np; ++jp) {
+                    {      // O += P V of pair jp
                         const uint32_t g = g0 + jp;
                         const uint32_t st = g % VSTAGES, ph = (g / VSTAGES) & 1, pb = g % PBUFS;
                         const bool two = 2 * jp + 1 < it.nt;
